@@ -1,0 +1,136 @@
+/*
+ * prism.h -- C ABI of libprism_b200.so: the data-parallel hot path of PRISM STEM
+ * image simulation (arXiv 1706.08563, "Prismatic") on one NVIDIA B200 (sm_100a).
+ *
+ * Citations are to /root/reference/PAPER.md (line, section/equation) and to the
+ * readings R# recorded in DESIGN.md where the paper is silent.
+ *
+ * Units: lengths in Angstrom, angles in radian, voltage in volt.
+ * Arrays are row-major; "[a][b]" means b is contiguous.
+ * DFT convention: forward F[k] = sum_n x[n] exp(-2 pi i k n / N), inverse carries
+ * 1/N; array slot m holds signed frequency k = m (m < N/2) or m - N.
+ *
+ * Ownership: the caller owns every buffer (V, S, out, workspace) and the CUDA
+ * stream.  The library allocates no device memory, keeps no state between calls
+ * ("perform all memory allocations initially"), and enqueues its work
+ * on the given stream; outputs are valid once the caller has synchronised that
+ * stream.  Host-side tables are built in fp64 inside each call.  When a potential
+ * is streamed from host memory the library uses a private copy stream and events,
+ * created and released inside the call; all of its copies are joined into `stream`.
+ *
+ * Errors: every int-returning function returns PRISM_OK (0) or a negative code;
+ * nothing aborts, nothing throws across the ABI.  There is no CPU fallback: on a
+ * machine without a CUDA device the compute calls return PRISM_ECUDA.
+ */
+#ifndef PRISM_B200_H
+#define PRISM_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+    PRISM_OK           =  0,
+    PRISM_EINVAL       = -1,  /* null pointer, unsupported grid, f does not divide n, alpha beyond the band-limit, ... */
+    PRISM_ENOMEM       = -2,  /* workspace too small (ask prism_workspace_bytes)                                      */
+    PRISM_ECUDA        = -3,  /* a CUDA call failed; prism_last_error() holds the CUDA message                        */
+    PRISM_EUNSUPPORTED = -4,  /* valid request outside what this build covers (e.g. window larger than 128 x 128)    */
+    PRISM_ENOLUT       = -5   /* an atom's Z has no lookup table                                                     */
+};
+
+/* The paper's parameters (cell & pixel size PAPER.md:158,:182; slice thickness :158,:200; voltage :182;
+ * probe semi-angle :200,:214; interpolation factor f :86; probe grid/step :174,:200; batch_size :126;
+ * memory mode :138; annular detectors :82). */
+typedef struct prism_params {
+    double  cell[3];            /* lx, ly, lz                                                              */
+    int32_t nx, ny;             /* grid; pixel = cell / n; powers of two in [64, 2048]                      */
+    double  slice_thickness;    /* t of Eq. (2)                                                             */
+    int32_t n_slices;           /* S (>= 1); atoms beyond the last slice are clamped into it (R14)          */
+    double  voltage;            /* -> lambda, sigma (relativistic closed forms, fp64; R0)                   */
+    double  alpha;              /* probe semi-angle; hard aperture edge, '<=' (R4)                          */
+    double  defocus, cs;        /* C1, C3: chi(q) = pi lambda q^2 C1 + (pi/2) C3 lambda^3 q^4, probe carries exp(-i chi) (R5) */
+    int32_t f;                  /* PRISM interpolation factor; must divide nx and ny; window = n / f (R8)    */
+    int32_t probes_x, probes_y; /* probe grid; probe (ix, iy) sits at origin + (ix, iy) * step (R10)         */
+    double  probe_origin[2];
+    double  probe_step[2];
+    double  det_step, det_max;  /* annular ring width and outer angle; n_bins = round(det_max / det_step)    */
+    int32_t batch;              /* waves per batch: beams in prism_compute_smatrix, probes in
+                                   multislice_compute_output and prism_compute_output; 0 = library default.
+                                   Results do not depend on it (PAPER.md:126 batch_size).                   */
+    int32_t potential_on_host;  /* 0: V is device memory.  1: V is page-locked host memory and is streamed
+                                   slice by slice over a private copy stream.            */
+} prism_params;
+
+/* Per-species radial table of the projected atomic potential ("precomputed lookup table for
+ * each atom type", :116): v[i] = v_Z(r_i), r_i = i * r_cut / (n - 1); v_Z is the piecewise-linear
+ * interpolant, 0 beyond r_cut (inclusive cut).  v is HOST memory. */
+typedef struct prism_lut {
+    int32_t      z;
+    int32_t      n;
+    double       r_cut;
+    const float* v;
+} prism_lut;
+
+/* which = */
+enum { PRISM_WS_SMATRIX = 0, PRISM_WS_OUTPUT = 1, PRISM_WS_MULTISLICE = 2, PRISM_WS_POTENTIAL = 3 };
+
+/* Bytes of DEVICE workspace the corresponding call needs for these parameters (host-only, no CUDA). */
+size_t  prism_workspace_bytes(const prism_params* p, int32_t which);
+/* n_bins = round(det_max / det_step) (host-only). */
+int32_t prism_num_bins(const prism_params* p);
+/* Number of PRISM beams ("every f-th plane wave in both spatial dimensions inside the maximum
+ * scattering angle"): signed indices kx = 0 mod f, ky = 0 mod f with (kx/lx)^2 + (ky/ly)^2 <= (alpha/lambda)^2,
+ * decided in fp64 on the host. */
+int     prism_num_beams(const prism_params* p, int32_t* n_beams);
+/* lambda (Angstrom) and sigma (rad / (V Angstrom)) used by the library for this voltage (host-only). */
+int     prism_constants(double voltage, double* lambda, double* sigma);
+
+/* Projected potential (Fig. 1a-b).  For every atom, slice s = clamp(floor(z / t)); every
+ * pixel within r_cut of the atom (exact sub-pixel distance, periodic in x and y) receives v_Z(r).
+ *   atoms_xyz  HOST  [n_atoms][3] fp64        z_number  HOST [n_atoms]        luts  HOST [n_luts]
+ *   v          OUT   [n_slices][ny][nx] fp32: device memory, or page-locked host memory if potential_on_host
+ *   workspace  DEVICE, prism_workspace_bytes(p, PRISM_WS_POTENTIAL) + 32 bytes per atom
+ * Deterministic (gather, fixed summation order).  Requires 2 r_cut < lx, ly. */
+int prism_build_potential(const prism_params* p, const double* atoms_xyz, const int32_t* z_number,
+                          int64_t n_atoms, const prism_lut* luts, int32_t n_luts, float* v,
+                          void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* Compact S-matrix (Fig. 1g-h): every beam's plane wave exp(+2 pi i q_b . r) is taken
+ * through all slices, psi <- IFFT2[ P . FFT2[ psi . exp(i sigma V_s) ] ] (Eq. 1, Eq. 2 with the 2/3
+ * band-limit on P), and its real-space exit wave stored as layer b at full resolution (R17).
+ *   v      IN   [n_slices][ny][nx] fp32, device or page-locked host (potential_on_host)
+ *   beams  OUT  HOST [n_beams][2] int32 (kx, ky) of each layer, n_beams from prism_num_beams
+ *   s      OUT  DEVICE complex64 [n_beams][ny][nx]; also the working set (waves are updated in place)
+ *   workspace DEVICE, prism_workspace_bytes(p, PRISM_WS_SMATRIX) */
+int prism_compute_smatrix(const prism_params* p, const float* v, int32_t* beams, void* s,
+                          void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* PRISM probes (Fig. 1i-k): for every probe of the grid, the (nx/f) x (ny/f) window of
+ * every layer around the probe is weighted by A_b exp(-i chi_b) exp(-2 pi i q_b . r_p) / (sqrt(n_beams)
+ * sqrt(mx my)) and summed over beams, Fourier transformed, squared (/ (mx my)) and integrated into rings.
+ *   s      IN   DEVICE complex64 [n_beams][ny][nx]      beams  IN  HOST [n_beams][2]
+ *   out    OUT  fp32 [probes_y][probes_x][n_bins]; device memory or host memory (then copied inside the call)
+ *   workspace DEVICE, prism_workspace_bytes(p, PRISM_WS_OUTPUT) */
+int prism_compute_output(const prism_params* p, const void* s, const int32_t* beams, int32_t n_beams,
+                         float* out, void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* Conventional multislice (Fig. 1c-e), the comparison path: every probe of the grid
+ * is built in Fourier space (hard aperture, exp(-i chi), position phase; sum |psi0|^2 = 1), taken through
+ * all slices by the same kernels, and |FFT2(psi_S)|^2 / (nx ny) is integrated into rings.
+ *   v, out, workspace as above (workspace: PRISM_WS_MULTISLICE). */
+int multislice_compute_output(const prism_params* p, const float* v, float* out,
+                              void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* Text for an error code, and the message of the last CUDA failure seen by the calling thread. */
+const char* prism_strerror(int code);
+const char* prism_last_error(void);
+/* Kernel launches enqueued by the calling thread since the last reset (for launch accounting). */
+int64_t prism_launch_count(int32_t reset);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PRISM_B200_H */

@@ -1,0 +1,847 @@
+// api.cu -- the C ABI of include/prism.h: parameter checks, fp64 host tables, workspace
+// layout and the drivers that enqueue the kernels (B2 "drivers" of SURVEY.md section 1).
+//
+// Everything that decides an integer (beam membership, band-limit, detector ring of a
+// pixel, window origin) is decided here in fp64 and handed to the kernels as tables.
+#include <algorithm>
+#include <atomic>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <vector>
+
+#include "../../include/prism.h"
+#include "prism_internal.h"
+
+namespace prism {
+
+static thread_local char g_last_error[512] = "";
+static std::atomic<long long> g_launches{0};
+
+static int cuda_fail(cudaError_t e, const char* what)
+{
+    snprintf(g_last_error, sizeof(g_last_error), "%s: %s", what, cudaGetErrorString(e));
+    return PRISM_ECUDA;
+}
+#define CU(call)                                                    \
+    do {                                                            \
+        cudaError_t e__ = (call);                                   \
+        if (e__ != cudaSuccess) return cuda_fail(e__, #call);       \
+    } while (0)
+#define LAUNCH(call)                                                \
+    do {                                                            \
+        cudaError_t e__ = (call);                                   \
+        if (e__ != cudaSuccess) return cuda_fail(e__, #call);       \
+        g_launches.fetch_add(1, std::memory_order_relaxed);         \
+    } while (0)
+
+static const double kPi = 3.14159265358979323846264338327950288;
+
+// ---- physics constants (R0): lambda = h / p, sigma = 2 pi gamma m e lambda / h^2 ----------------
+static void electron_constants(double volt, double* lambda_a, double* sigma)
+{
+    const double h = 6.62607015e-34, c = 299792458.0, e = 1.602176634e-19, m = 9.1093837015e-31;
+    const double mc2 = m * c * c, ev = e * volt;
+    const double pc = std::sqrt(ev * (ev + 2.0 * mc2));          // momentum * c
+    const double lam_m = h * c / pc;
+    const double gamma = 1.0 + ev / mc2;
+    if (lambda_a) *lambda_a = lam_m * 1e10;
+    if (sigma) *sigma = 2.0 * kPi * gamma * m * e * lam_m / (h * h) * 1e-10;
+}
+
+static bool is_pow2(int n) { return n > 0 && (n & (n - 1)) == 0; }
+static int  signed_freq(int slot, int n) { return slot < n / 2 ? slot : slot - n; }
+
+static int check_common(const prism_params* p)
+{
+    if (!p) return PRISM_EINVAL;
+    if (!is_pow2(p->nx) || !is_pow2(p->ny) || p->nx < 64 || p->ny < 64 || p->nx > 2048 || p->ny > 2048) return PRISM_EINVAL;
+    if (!(p->cell[0] > 0) || !(p->cell[1] > 0) || !(p->slice_thickness > 0) || p->n_slices < 1) return PRISM_EINVAL;
+    if (!(p->voltage > 0)) return PRISM_EINVAL;
+    return PRISM_OK;
+}
+static int check_probe(const prism_params* p)
+{
+    if (!(p->alpha > 0) || p->probes_x < 1 || p->probes_y < 1) return PRISM_EINVAL;
+    if (!(p->det_step > 0) || !(p->det_max > 0) || prism_num_bins(p) < 1 || prism_num_bins(p) > 4096) return PRISM_EINVAL;
+    double lambda;
+    electron_constants(p->voltage, &lambda, nullptr);
+    const double qnyq = std::min(p->nx / (2.0 * p->cell[0]), p->ny / (2.0 * p->cell[1]));
+    if (p->alpha / lambda >= 2.0 / 3.0 * qnyq) return PRISM_EINVAL;      // aperture must sit inside the band-limit
+    return PRISM_OK;
+}
+static int check_prism(const prism_params* p)
+{
+    if (p->f < 1 || p->nx % p->f || p->ny % p->f) return PRISM_EINVAL;
+    const int mx = p->nx / p->f, my = p->ny / p->f;
+    if (!is_pow2(mx) || !is_pow2(my)) return PRISM_EINVAL;
+    if (mx < 16 || my < 16) return PRISM_EUNSUPPORTED;
+    if (mx * my > 128 * 128) return PRISM_EUNSUPPORTED;
+    return PRISM_OK;
+}
+
+// ---- beams (R4, R7) -----------------------------------------------------------------
+static void list_beams(const prism_params* p, std::vector<int32_t>& beams)
+{
+    double lambda;
+    electron_constants(p->voltage, &lambda, nullptr);
+    const double qmax = p->alpha / lambda;
+    beams.clear();
+    for (int ky = -p->ny / 2; ky < p->ny / 2; ++ky) {
+        if (ky % p->f) continue;
+        for (int kx = -p->nx / 2; kx < p->nx / 2; ++kx) {
+            if (kx % p->f) continue;
+            const double qx = kx / p->cell[0], qy = ky / p->cell[1];
+            if (qx * qx + qy * qy <= qmax * qmax) { beams.push_back(kx); beams.push_back(ky); }
+        }
+    }
+}
+
+// ---- host tables ---------------------------------------------------------------------------------
+static void twiddle_table(int n, std::vector<float2>& tw)
+{
+    tw.resize(n);
+    for (int m = 0; m < n; ++m) {
+        const double a = -2.0 * kPi * (double)m / (double)n;
+        tw[m] = make_float2((float)std::cos(a), (float)std::sin(a));
+    }
+}
+
+// separable Fresnel propagator (Eq. 2), with an extra real factor folded in
+static void propagator_factor(int n, double length, double lambda, double dz, double extra, std::vector<float2>& out)
+{
+    out.resize(n);
+    for (int m = 0; m < n; ++m) {
+        const double q = signed_freq(m, n) / length;
+        const double a = -kPi * lambda * dz * q * q;
+        out[m] = make_float2((float)(extra * std::cos(a)), (float)(extra * std::sin(a)));
+    }
+}
+
+// 2/3 band-limit (R1): for every kx slot the largest |ky| with q^2 < (2/3 q_nyq)^2, -1 if none
+static void band_limit(const prism_params* p, std::vector<int>& ky_lim)
+{
+    const double qnyq = std::min(p->nx / (2.0 * p->cell[0]), p->ny / (2.0 * p->cell[1]));
+    const double qcut2 = (2.0 / 3.0 * qnyq) * (2.0 / 3.0 * qnyq);
+    ky_lim.assign(p->nx, -1);
+    for (int m = 0; m < p->nx; ++m) {
+        const double qx = signed_freq(m, p->nx) / p->cell[0];
+        for (int ky = 0; ky <= p->ny / 2; ++ky) {
+            const double qy = ky / p->cell[1];
+            if (qx * qx + qy * qy < qcut2) ky_lim[m] = ky; else break;
+        }
+    }
+}
+
+static double aberration(const prism_params* p, double lambda, double q2)
+{
+    return kPi * lambda * q2 * p->defocus + 0.5 * kPi * p->cs * lambda * lambda * lambda * q2 * q2;
+}
+
+// exp(-2 pi i k pos / length) for every probe coordinate and every listed index k
+static void position_phases(int n_probes, double origin, double step, double length,
+                            const std::vector<int>& ks, std::vector<float2>& out)
+{
+    out.resize((size_t)n_probes * ks.size());
+    for (int ip = 0; ip < n_probes; ++ip) {
+        const double pos = origin + ip * step;
+        for (size_t i = 0; i < ks.size(); ++i) {
+            double turns = ks[i] * (pos / length);
+            turns -= std::floor(turns);
+            const double a = -2.0 * kPi * turns;
+            out[(size_t)ip * ks.size() + i] = make_float2((float)std::cos(a), (float)std::sin(a));
+        }
+    }
+}
+
+// detector rings (R11): CSR lists of pixel indices per ring for an (my x mx) pattern whose slot
+// (ky, kx) is stored TRANSPOSED at kx * my + ky and has frequency (kx fx / lx, ky fy / ly).
+static void ring_lists(const prism_params* p, int mx, int my, int fx, int fy,
+                       std::vector<int>& start, std::vector<int>& pix)
+{
+    double lambda;
+    electron_constants(p->voltage, &lambda, nullptr);
+    const int nb = prism_num_bins(p);
+    std::vector<int> bin((size_t)mx * my);
+    std::vector<int> count(nb + 1, 0);
+    const double ilx2 = 1.0 / (p->cell[0] * p->cell[0]), ily2 = 1.0 / (p->cell[1] * p->cell[1]);
+    for (int sx = 0; sx < mx; ++sx) {
+        for (int sy = 0; sy < my; ++sy) {
+            const double kx = (double)(signed_freq(sx, mx) * fx), ky = (double)(signed_freq(sy, my) * fy);
+            const double q = std::sqrt(kx * kx * ilx2 + ky * ky * ily2);
+            const double angle = lambda * q;
+            const int b = (int)std::floor(angle / p->det_step);
+            bin[(size_t)sx * my + sy] = (b < nb) ? b : -1;
+            if (b < nb) ++count[b + 1];
+        }
+    }
+    start.assign(nb + 1, 0);
+    for (int b = 0; b < nb; ++b) start[b + 1] = start[b] + count[b + 1];
+    pix.resize(start[nb]);
+    std::vector<int> fill(start.begin(), start.end() - 1);
+    for (size_t i = 0; i < bin.size(); ++i)
+        if (bin[i] >= 0) pix[fill[bin[i]]++] = (int)i;
+}
+
+// ---- workspace bump allocator ----------------------------------------------------------------------
+struct Arena {
+    char*  base;
+    size_t size, used;
+    Arena(void* b, size_t s) : base((char*)b), size(s), used(0) {}
+    template <class T> T* take(size_t count)
+    {
+        const size_t bytes = (count * sizeof(T) + 255) / 256 * 256;
+        T* ptr = base ? (T*)(base + used) : nullptr;
+        used += bytes;
+        return ptr;
+    }
+    bool ok() const { return used <= size; }
+};
+
+template <class T>
+static cudaError_t upload(T* dst, const std::vector<T>& src, cudaStream_t st)
+{
+    if (src.empty()) return cudaSuccess;
+    return cudaMemcpyAsync(dst, src.data(), src.size() * sizeof(T), cudaMemcpyHostToDevice, st);
+}
+
+static int default_probe_batch(const prism_params* p, size_t bytes_per_probe)
+{
+    long long n = (long long)p->probes_x * p->probes_y;
+    // default: about 4 GiB of waves per batch (enough to hide a streamed potential behind the passes)
+    long long b = p->batch > 0 ? p->batch : std::max<long long>(1, (long long)(4ull << 30) / (long long)bytes_per_probe);
+    return (int)std::min(n, b);
+}
+
+// ---- potential slices: resident, or streamed from page-locked host memory -------
+// A ring of RING raw slices is filled over a private copy stream; the (tiny) transmission kernel
+// turns the slice into t_s = exp(i sigma V_s) on the main stream and frees the ring slot.
+struct SliceFeeder {
+    static constexpr int RING = 3;
+    const float* v = nullptr;
+    bool on_host = false;
+    int64_t npix = 0;
+    int n_slices = 0;
+    double sigma = 0;
+    float2* tbuf = nullptr;
+    float* ring[RING] = {nullptr, nullptr, nullptr};
+    cudaStream_t main_stream = nullptr, copy_stream = nullptr;
+    cudaEvent_t filled[RING] = {}, consumed[RING] = {};
+    bool slot_used[RING] = {false, false, false};
+    int next_copy = 0;
+
+    int init()
+    {
+        if (!on_host) return PRISM_OK;
+        CU(cudaStreamCreateWithFlags(&copy_stream, cudaStreamNonBlocking));
+        for (int r = 0; r < RING; ++r) {
+            CU(cudaEventCreateWithFlags(&filled[r], cudaEventDisableTiming));
+            CU(cudaEventCreateWithFlags(&consumed[r], cudaEventDisableTiming));
+        }
+        // copies must not start before earlier work on the main stream that may still use the ring
+        cudaEvent_t start;
+        CU(cudaEventCreateWithFlags(&start, cudaEventDisableTiming));
+        CU(cudaEventRecord(start, main_stream));
+        CU(cudaStreamWaitEvent(copy_stream, start, 0));
+        CU(cudaEventDestroy(start));
+        return PRISM_OK;
+    }
+    void begin_sweep() { next_copy = 0; }
+    int prefetch(int upto)
+    {
+        for (; next_copy < std::min(n_slices, upto); ++next_copy) {
+            const int r = next_copy % RING;
+            if (slot_used[r]) CU(cudaStreamWaitEvent(copy_stream, consumed[r], 0));
+            CU(cudaMemcpyAsync(ring[r], v + (size_t)next_copy * npix, npix * sizeof(float),
+                               cudaMemcpyHostToDevice, copy_stream));
+            CU(cudaEventRecord(filled[r], copy_stream));
+            slot_used[r] = true;
+        }
+        return PRISM_OK;
+    }
+    // enqueue everything needed so that tbuf holds t_s for the kernels enqueued next on main_stream
+    int get(int s)
+    {
+        const float* src = v + (size_t)s * npix;
+        if (on_host) {
+            int rc = prefetch(s + RING);
+            if (rc) return rc;
+            const int r = s % RING;
+            CU(cudaStreamWaitEvent(main_stream, filled[r], 0));
+            src = ring[r];
+        }
+        LAUNCH(launch_transmission(src, tbuf, sigma, npix, main_stream));
+        if (on_host) CU(cudaEventRecord(consumed[s % RING], main_stream));
+        return PRISM_OK;
+    }
+    void release()
+    {
+        if (!on_host) return;
+        for (int r = 0; r < RING; ++r) {
+            if (filled[r]) cudaEventDestroy(filled[r]);
+            if (consumed[r]) cudaEventDestroy(consumed[r]);
+        }
+        if (copy_stream) cudaStreamDestroy(copy_stream);
+    }
+};
+
+// tables every slice loop needs
+struct SliceTables {
+    float2 *tw_x, *tw_y, *prop_x, *prop_y;
+    int* ky_lim;
+};
+static void carve_slice_tables(Arena& a, const prism_params* p, SliceTables& t)
+{
+    t.tw_x = a.take<float2>(p->nx);
+    t.tw_y = a.take<float2>(p->ny);
+    t.prop_x = a.take<float2>(p->nx);
+    t.prop_y = a.take<float2>(p->ny);
+    t.ky_lim = a.take<int>(p->nx);
+}
+static int fill_slice_tables(const prism_params* p, const SliceTables& t, cudaStream_t st)
+{
+    double lambda;
+    electron_constants(p->voltage, &lambda, nullptr);
+    std::vector<float2> h;
+    twiddle_table(p->nx, h);
+    CU(upload(t.tw_x, h, st));
+    twiddle_table(p->ny, h);
+    CU(upload(t.tw_y, h, st));
+    // the row pass runs unscaled inverse FFTs and so does the column pass: fold 1/nx and 1/ny here
+    propagator_factor(p->nx, p->cell[0], lambda, p->slice_thickness, 1.0 / p->nx, h);
+    CU(upload(t.prop_x, h, st));
+    propagator_factor(p->ny, p->cell[1], lambda, p->slice_thickness, 1.0 / p->ny, h);
+    CU(upload(t.prop_y, h, st));
+    std::vector<int> lim;
+    band_limit(p, lim);
+    CU(upload(t.ky_lim, lim, st));
+    return PRISM_OK;
+}
+static void carve_feeder(Arena& a, const prism_params* p, SliceFeeder& f)
+{
+    const size_t npix = (size_t)p->nx * p->ny;
+    f.tbuf = a.take<float2>(npix);
+    if (p->potential_on_host)
+        for (int r = 0; r < SliceFeeder::RING; ++r) f.ring[r] = a.take<float>(npix);
+}
+
+// ---- layouts -----------------------------------------------------------------------------------------
+struct SmatrixLayout { SliceTables tab; SliceFeeder feed; int2* beams; };
+static void layout_smatrix(Arena& a, const prism_params* p, int n_beams, SmatrixLayout& L)
+{
+    carve_slice_tables(a, p, L.tab);
+    carve_feeder(a, p, L.feed);
+    L.beams = a.take<int2>(n_beams);
+}
+
+struct OutputLayout {
+    float2 *tw_x, *tw_y, *coef_b, *phase_x, *phase_y, *w;
+    int *win_x0, *win_y0, *bin_start, *bin_pix;
+    float *intensity, *out_stage;
+    int batch;
+};
+static void layout_output(Arena& a, const prism_params* p, int n_beams, OutputLayout& L)
+{
+    const int mx = p->nx / p->f, my = p->ny / p->f, nb = prism_num_bins(p);
+    const size_t npix = (size_t)mx * my;
+    L.batch = default_probe_batch(p, npix * 12);
+    L.tw_x = a.take<float2>(mx);
+    L.tw_y = a.take<float2>(my);
+    L.coef_b = a.take<float2>(n_beams);
+    L.phase_x = a.take<float2>((size_t)p->probes_x * n_beams);
+    L.phase_y = a.take<float2>((size_t)p->probes_y * n_beams);
+    L.win_x0 = a.take<int>(p->probes_x);
+    L.win_y0 = a.take<int>(p->probes_y);
+    L.bin_start = a.take<int>(nb + 1);
+    L.bin_pix = a.take<int>(npix);
+    L.w = a.take<float2>((size_t)L.batch * npix);
+    L.intensity = a.take<float>((size_t)L.batch * npix);
+    L.out_stage = a.take<float>((size_t)p->probes_x * p->probes_y * nb);
+}
+
+struct MultisliceLayout {
+    SliceTables tab;
+    SliceFeeder feed;
+    float2 *aperture_t, *phase_x, *phase_y, *psi;
+    int *bin_start, *bin_pix;
+    float *intensity, *out_stage;
+    int batch;
+};
+static void layout_multislice(Arena& a, const prism_params* p, MultisliceLayout& L)
+{
+    const size_t npix = (size_t)p->nx * p->ny;
+    const int nb = prism_num_bins(p);
+    L.batch = default_probe_batch(p, npix * 12);
+    carve_slice_tables(a, p, L.tab);
+    carve_feeder(a, p, L.feed);
+    L.aperture_t = a.take<float2>(npix);
+    L.phase_x = a.take<float2>((size_t)p->probes_x * p->nx);
+    L.phase_y = a.take<float2>((size_t)p->probes_y * p->ny);
+    L.bin_start = a.take<int>(nb + 1);
+    L.bin_pix = a.take<int>(npix);
+    L.psi = a.take<float2>((size_t)L.batch * npix);
+    L.intensity = a.take<float>((size_t)L.batch * npix);
+    L.out_stage = a.take<float>((size_t)p->probes_x * p->probes_y * nb);
+}
+
+constexpr int POT_TILE = 16;
+constexpr int POT_CHUNK_SLICES = 8;
+struct PotentialLayout { int* cell_start; float* lut_v; double* lut_rcut; float* stage; };
+static void layout_potential(Arena& a, const prism_params* p, int n_luts, int lut_n, PotentialLayout& L)
+{
+    const size_t cells = (size_t)p->n_slices * (p->nx / POT_TILE) * (p->ny / POT_TILE);
+    L.cell_start = a.take<int>(cells + 1);
+    L.lut_v = a.take<float>((size_t)std::max(1, n_luts) * std::max(2, lut_n));
+    L.lut_rcut = a.take<double>(std::max(1, n_luts));
+    L.stage = p->potential_on_host ? a.take<float>((size_t)POT_CHUNK_SLICES * p->nx * p->ny) : nullptr;
+}
+
+static bool pointer_is_device(const void* ptr)
+{
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, ptr) != cudaSuccess) { cudaGetLastError(); return false; }
+    return at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged;
+}
+
+}  // namespace prism
+
+using namespace prism;
+
+// =========================================================================================================
+extern "C" {
+#pragma GCC visibility push(default)
+
+const char* prism_strerror(int code)
+{
+    switch (code) {
+        case PRISM_OK: return "ok";
+        case PRISM_EINVAL: return "invalid argument";
+        case PRISM_ENOMEM: return "workspace too small";
+        case PRISM_ECUDA: return "CUDA error";
+        case PRISM_EUNSUPPORTED: return "unsupported configuration";
+        case PRISM_ENOLUT: return "no lookup table for an atom's Z";
+    }
+    return "unknown error";
+}
+const char* prism_last_error(void) { return g_last_error; }
+
+int64_t prism_launch_count(int32_t reset)
+{
+    return reset ? g_launches.exchange(0) : g_launches.load();
+}
+
+int prism_constants(double voltage, double* lambda, double* sigma)
+{
+    if (!(voltage > 0)) return PRISM_EINVAL;
+    electron_constants(voltage, lambda, sigma);
+    return PRISM_OK;
+}
+
+int32_t prism_num_bins(const prism_params* p)
+{
+    if (!p || !(p->det_step > 0)) return 0;
+    return (int32_t)std::floor(p->det_max / p->det_step + 0.5);
+}
+
+int prism_num_beams(const prism_params* p, int32_t* n_beams)
+{
+    if (!n_beams) return PRISM_EINVAL;
+    int rc = check_common(p);
+    if (rc) return rc;
+    if ((rc = check_probe(p))) return rc;
+    if (p->f < 1 || p->nx % p->f || p->ny % p->f) return PRISM_EINVAL;
+    std::vector<int32_t> beams;
+    list_beams(p, beams);
+    *n_beams = (int32_t)(beams.size() / 2);
+    return PRISM_OK;
+}
+
+size_t prism_workspace_bytes(const prism_params* p, int32_t which)
+{
+    if (check_common(p)) return 0;
+    Arena a(nullptr, 0);
+    switch (which) {
+        case PRISM_WS_SMATRIX: {
+            int32_t nb = 0;
+            if (prism_num_beams(p, &nb)) return 0;
+            SmatrixLayout L;
+            layout_smatrix(a, p, nb, L);
+            break;
+        }
+        case PRISM_WS_OUTPUT: {
+            int32_t nb = 0;
+            if (prism_num_beams(p, &nb) || check_prism(p)) return 0;
+            OutputLayout L;
+            layout_output(a, p, nb, L);
+            break;
+        }
+        case PRISM_WS_MULTISLICE: {
+            if (check_probe(p)) return 0;
+            MultisliceLayout L;
+            layout_multislice(a, p, L);
+            break;
+        }
+        case PRISM_WS_POTENTIAL: {
+            PotentialLayout L;
+            layout_potential(a, p, 128, 4096, L);       // room for 128 species x 4096 samples; atoms are extra
+            break;
+        }
+        default: return 0;
+    }
+    return a.used + 256;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+int prism_build_potential(const prism_params* p, const double* atoms_xyz, const int32_t* z_number,
+                          int64_t n_atoms, const prism_lut* luts, int32_t n_luts, float* v,
+                          void* workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    int rc = check_common(p);
+    if (rc) return rc;
+    if (n_atoms < 0 || (n_atoms > 0 && (!atoms_xyz || !z_number)) || !v || !workspace) return PRISM_EINVAL;
+    if (n_luts < 0 || n_luts > 128 || (n_atoms > 0 && (n_luts == 0 || !luts))) return PRISM_EINVAL;
+    if (n_atoms > (int64_t)0x7fffffff) return PRISM_EUNSUPPORTED;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int lut_n = 2;
+    double rc_max = 0.0;
+    for (int l = 0; l < n_luts; ++l) {
+        if (!luts[l].v || luts[l].n < 2 || luts[l].n > 4096 || !(luts[l].r_cut > 0)) return PRISM_EINVAL;
+        if (l > 0 && luts[l].n != luts[0].n) return PRISM_EUNSUPPORTED;       // one table length per call
+        lut_n = luts[l].n;
+        rc_max = std::max(rc_max, luts[l].r_cut);
+    }
+    if (2.0 * rc_max >= p->cell[0] || 2.0 * rc_max >= p->cell[1]) return PRISM_EINVAL;
+
+    const int nx = p->nx, ny = p->ny, ns = p->n_slices;
+    const int tiles_x = nx / POT_TILE, tiles_y = ny / POT_TILE;
+    const double px = p->cell[0] / nx, py = p->cell[1] / ny;
+    const size_t cells = (size_t)ns * tiles_x * tiles_y;
+
+    Arena a(workspace, workspace_bytes);
+    PotentialLayout L;
+    layout_potential(a, p, 128, 4096, L);
+    PotAtom* d_atoms = a.take<PotAtom>((size_t)n_atoms);
+    if (!a.ok()) return PRISM_ENOMEM;
+
+    // host: slice + tile of every atom, counting sort by cell (stable: original order inside a cell)
+    std::vector<int> cell_of((size_t)n_atoms);
+    std::vector<int> start(cells + 1, 0);
+    std::vector<PotAtom> sorted((size_t)n_atoms);
+    std::vector<PotAtom> tmp((size_t)n_atoms);
+    for (int64_t i = 0; i < n_atoms; ++i) {
+        int lut = -1;
+        for (int l = 0; l < n_luts; ++l) if (luts[l].z == z_number[i]) lut = l;
+        if (lut < 0) return PRISM_ENOLUT;
+        double x = atoms_xyz[3 * i], y = atoms_xyz[3 * i + 1], z = atoms_xyz[3 * i + 2];
+        x -= p->cell[0] * std::floor(x / p->cell[0]);
+        y -= p->cell[1] * std::floor(y / p->cell[1]);
+        int s = (int)std::floor(z / p->slice_thickness);
+        s = std::min(std::max(s, 0), ns - 1);
+        int ix = std::min(std::max((int)std::floor(x / px), 0), nx - 1);
+        int iy = std::min(std::max((int)std::floor(y / py), 0), ny - 1);
+        const int cell = (s * tiles_y + iy / POT_TILE) * tiles_x + ix / POT_TILE;
+        cell_of[i] = cell;
+        ++start[cell + 1];
+        tmp[i].x = x; tmp[i].y = y; tmp[i].lut = lut; tmp[i].pad = 0;
+    }
+    for (size_t c = 0; c < cells; ++c) start[c + 1] += start[c];
+    {
+        std::vector<int> fill(start.begin(), start.end() - 1);
+        for (int64_t i = 0; i < n_atoms; ++i) sorted[fill[cell_of[i]]++] = tmp[i];
+    }
+    std::vector<float> h_lut((size_t)std::max(1, n_luts) * lut_n, 0.f);
+    std::vector<double> h_rcut(std::max(1, n_luts), 1.0);
+    for (int l = 0; l < n_luts; ++l) {
+        std::memcpy(&h_lut[(size_t)l * lut_n], luts[l].v, sizeof(float) * lut_n);
+        h_rcut[l] = luts[l].r_cut;
+    }
+    CU(upload(L.cell_start, start, st));
+    CU(upload(L.lut_v, h_lut, st));
+    CU(upload(L.lut_rcut, h_rcut, st));
+    CU(upload(d_atoms, sorted, st));
+
+    PotentialArgs g;
+    g.atoms = d_atoms; g.cell_start = L.cell_start; g.lut_v = L.lut_v; g.lut_rcut = L.lut_rcut; g.lut_n = lut_n;
+    g.nx = nx; g.ny = ny; g.tiles_x = tiles_x; g.tiles_y = tiles_y; g.tile = POT_TILE;
+    const double reach_px = std::max(rc_max / px, rc_max / py);
+    g.reach_tiles = (int)std::ceil(reach_px / POT_TILE);
+    g.px = px; g.py = py; g.lx = p->cell[0]; g.ly = p->cell[1];
+    const size_t npix = (size_t)nx * ny;
+    if (!p->potential_on_host) {
+        // grid.y is limited to 65535 slices per launch
+        for (int s0 = 0; s0 < ns; s0 += 32768) {
+            g.slice0 = s0; g.n_slices_chunk = std::min(32768, ns - s0); g.v_out = v + (size_t)s0 * npix;
+            LAUNCH(launch_potential(g, st));
+        }
+    } else {
+        for (int s0 = 0; s0 < ns; s0 += POT_CHUNK_SLICES) {
+            g.slice0 = s0; g.n_slices_chunk = std::min(POT_CHUNK_SLICES, ns - s0); g.v_out = L.stage;
+            LAUNCH(launch_potential(g, st));
+            CU(cudaMemcpyAsync(v + (size_t)s0 * npix, L.stage, (size_t)g.n_slices_chunk * npix * sizeof(float),
+                               cudaMemcpyDeviceToHost, st));
+        }
+    }
+    // the sorted host vectors die here: make sure the (pageable) uploads have been staged
+    CU(cudaStreamSynchronize(st));
+    return PRISM_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+int prism_compute_smatrix(const prism_params* p, const float* v, int32_t* beams_out, void* s,
+                          void* workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    int rc = check_common(p);
+    if (rc) return rc;
+    if ((rc = check_probe(p))) return rc;
+    if (p->f < 1 || p->nx % p->f || p->ny % p->f) return PRISM_EINVAL;
+    if (!v || !beams_out || !s || !workspace) return PRISM_EINVAL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+
+    std::vector<int32_t> beams;
+    list_beams(p, beams);
+    const int n_beams = (int)(beams.size() / 2);
+    std::memcpy(beams_out, beams.data(), beams.size() * sizeof(int32_t));
+
+    Arena a(workspace, workspace_bytes);
+    SmatrixLayout L;
+    layout_smatrix(a, p, n_beams, L);
+    if (!a.ok()) return PRISM_ENOMEM;
+    if ((rc = fill_slice_tables(p, L.tab, st))) return rc;
+    CU(cudaMemcpyAsync(L.beams, beams.data(), beams.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+    CU(cudaStreamSynchronize(st));          // `beams` (pageable) is local
+
+    double sigma;
+    electron_constants(p->voltage, nullptr, &sigma);
+    const size_t npix = (size_t)p->nx * p->ny;
+    SliceFeeder& feed = L.feed;
+    feed.v = v; feed.on_host = p->potential_on_host != 0; feed.npix = (int64_t)npix; feed.n_slices = p->n_slices;
+    feed.sigma = sigma; feed.main_stream = st;
+    if ((rc = feed.init())) { feed.release(); return rc; }
+
+    const int batch = p->batch > 0 ? std::min<int>(p->batch, n_beams) : n_beams;
+    auto run = [&]() -> int {
+        for (int b0 = 0; b0 < n_beams; b0 += batch) {
+            const int nb = std::min(batch, n_beams - b0);
+            RowArgs ra;
+            ra.a = (float2*)s + (size_t)b0 * npix; ra.out = ra.a; ra.t = feed.tbuf;
+            ra.tw_x = L.tab.tw_x; ra.tw_y = L.tab.tw_y; ra.beams = L.beams + b0;
+            ra.n_waves = nb; ra.nx = p->nx; ra.ny = p->ny; ra.scale = 1.f;
+            ColArgs ca;
+            std::memset(&ca, 0, sizeof(ca));
+            ca.a = ra.a; ca.tw_y = L.tab.tw_y; ca.prop_x = L.tab.prop_x; ca.prop_y = L.tab.prop_y;
+            ca.ky_lim = L.tab.ky_lim; ca.n_waves = nb; ca.nx = p->nx; ca.ny = p->ny; ca.scale = 1.f;
+            feed.begin_sweep();
+            for (int sl = 0; sl < p->n_slices; ++sl) {
+                int r = feed.get(sl);
+                if (r) return r;
+                if (sl == 0) {
+                    ra.scale = (float)p->nx;                 // keeps A' = nx * FFT_x(t psi), see DESIGN.md
+                    LAUNCH(launch_row_pass(ROW_INIT, ra, st));
+                } else {
+                    LAUNCH(launch_row_pass(ROW_STEP, ra, st));
+                }
+                LAUNCH(launch_col_pass(COL_STEP, ca, st));
+            }
+            ra.scale = 1.0f / (float)p->nx;
+            LAUNCH(launch_row_pass(ROW_FINAL, ra, st));
+        }
+        return PRISM_OK;
+    };
+    rc = run();
+    feed.release();
+    return rc;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+static int copy_out(const prism_params* p, float* out, float* stage, bool out_is_device, cudaStream_t st)
+{
+    if (out_is_device) return PRISM_OK;
+    const size_t bytes = (size_t)p->probes_x * p->probes_y * prism_num_bins(p) * sizeof(float);
+    CU(cudaMemcpyAsync(out, stage, bytes, cudaMemcpyDeviceToHost, st));
+    return PRISM_OK;
+}
+
+int prism_compute_output(const prism_params* p, const void* s, const int32_t* beams, int32_t n_beams,
+                         float* out, void* workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    int rc = check_common(p);
+    if (rc) return rc;
+    if ((rc = check_probe(p))) return rc;
+    if ((rc = check_prism(p))) return rc;
+    if (!s || !beams || n_beams < 1 || !out || !workspace) return PRISM_EINVAL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const int mx = p->nx / p->f, my = p->ny / p->f, nb = prism_num_bins(p);
+    const size_t npix = (size_t)mx * my;
+    double lambda;
+    electron_constants(p->voltage, &lambda, nullptr);
+
+    Arena a(workspace, workspace_bytes);
+    OutputLayout L;
+    layout_output(a, p, n_beams, L);
+    if (!a.ok()) return PRISM_ENOMEM;
+    const bool out_dev = pointer_is_device(out);
+    float* d_out = out_dev ? out : L.out_stage;
+
+    // host tables (fp64)
+    std::vector<float2> h;
+    twiddle_table(mx, h);
+    CU(upload(L.tw_x, h, st));
+    std::vector<float2> h2;
+    twiddle_table(my, h2);
+    CU(upload(L.tw_y, h2, st));
+    std::vector<int> kxs(n_beams), kys(n_beams);
+    std::vector<float2> coef(n_beams);
+    const double wscale = 1.0 / (std::sqrt((double)n_beams) * std::sqrt((double)npix));     // R6
+    for (int b = 0; b < n_beams; ++b) {
+        kxs[b] = beams[2 * b]; kys[b] = beams[2 * b + 1];
+        const double qx = kxs[b] / p->cell[0], qy = kys[b] / p->cell[1];
+        const double chi = aberration(p, lambda, qx * qx + qy * qy);
+        coef[b] = make_float2((float)(wscale * std::cos(-chi)), (float)(wscale * std::sin(-chi)));
+    }
+    CU(upload(L.coef_b, coef, st));
+    std::vector<float2> phx, phy;
+    position_phases(p->probes_x, p->probe_origin[0], p->probe_step[0], p->cell[0], kxs, phx);
+    position_phases(p->probes_y, p->probe_origin[1], p->probe_step[1], p->cell[1], kys, phy);
+    CU(upload(L.phase_x, phx, st));
+    CU(upload(L.phase_y, phy, st));
+    // window origin (R8): centre = round-half-up pixel, start = centre - M/2, periodic
+    std::vector<int> wx0(p->probes_x), wy0(p->probes_y);
+    const double px = p->cell[0] / p->nx, py = p->cell[1] / p->ny;
+    for (int i = 0; i < p->probes_x; ++i) {
+        const long long c = (long long)std::floor((p->probe_origin[0] + i * p->probe_step[0]) / px + 0.5);
+        wx0[i] = (int)((((c - mx / 2) % p->nx) + p->nx) % p->nx);
+    }
+    for (int i = 0; i < p->probes_y; ++i) {
+        const long long c = (long long)std::floor((p->probe_origin[1] + i * p->probe_step[1]) / py + 0.5);
+        wy0[i] = (int)((((c - my / 2) % p->ny) + p->ny) % p->ny);
+    }
+    CU(upload(L.win_x0, wx0, st));
+    CU(upload(L.win_y0, wy0, st));
+    std::vector<int> bstart, bpix;
+    ring_lists(p, mx, my, p->f, p->f, bstart, bpix);
+    CU(upload(L.bin_start, bstart, st));
+    CU(upload(L.bin_pix, bpix, st));
+    CU(cudaStreamSynchronize(st));          // host vectors above are local
+
+    const int n_probes = p->probes_x * p->probes_y;
+    for (int p0 = 0; p0 < n_probes; p0 += L.batch) {
+        const int np = std::min(L.batch, n_probes - p0);
+        BeamSumArgs g;
+        g.s = (const float2*)s; g.w = L.w; g.coef_b = L.coef_b; g.phase_x = L.phase_x; g.phase_y = L.phase_y;
+        g.win_x0 = L.win_x0; g.win_y0 = L.win_y0; g.n_beams = n_beams; g.nx = p->nx; g.ny = p->ny;
+        g.mx = mx; g.my = my; g.probe0 = p0; g.n_probes_batch = np; g.probes_x = p->probes_x;
+        LAUNCH(launch_beam_sum(g, st));
+        RowArgs ra;
+        std::memset(&ra, 0, sizeof(ra));
+        ra.a = L.w; ra.out = L.w; ra.tw_x = L.tw_x; ra.tw_y = L.tw_y; ra.n_waves = np; ra.nx = mx; ra.ny = my; ra.scale = 1.f;
+        LAUNCH(launch_row_pass(ROW_FFT, ra, st));
+        ColArgs ca;
+        std::memset(&ca, 0, sizeof(ca));
+        ca.a = L.w; ca.intensity = L.intensity; ca.tw_y = L.tw_y; ca.n_waves = np; ca.nx = mx; ca.ny = my;
+        ca.scale = (float)(1.0 / (double)npix);
+        LAUNCH(launch_col_pass(COL_ABS2, ca, st));
+        LAUNCH(launch_bin_reduce(L.intensity, (int64_t)npix, L.bin_start, L.bin_pix, nb,
+                                 d_out + (size_t)p0 * nb, np, st));
+    }
+    return copy_out(p, out, L.out_stage, out_dev, st);
+}
+
+// ---------------------------------------------------------------------------------------------------------
+int multislice_compute_output(const prism_params* p, const float* v, float* out,
+                              void* workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    int rc = check_common(p);
+    if (rc) return rc;
+    if ((rc = check_probe(p))) return rc;
+    if (!v || !out || !workspace) return PRISM_EINVAL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const int nx = p->nx, ny = p->ny, nb = prism_num_bins(p);
+    const size_t npix = (size_t)nx * ny;
+    double lambda, sigma;
+    electron_constants(p->voltage, &lambda, &sigma);
+
+    Arena a(workspace, workspace_bytes);
+    MultisliceLayout L;
+    layout_multislice(a, p, L);
+    if (!a.ok()) return PRISM_ENOMEM;
+    const bool out_dev = pointer_is_device(out);
+    float* d_out = out_dev ? out : L.out_stage;
+
+    if ((rc = fill_slice_tables(p, L.tab, st))) return rc;
+    // probe spectrum (R4-R6): A_k exp(-i chi_k) * sqrt(nx ny) / sqrt(N_A), with the 1/ny of the
+    // unscaled inverse column transform folded in; stored transposed [kx][ky]
+    std::vector<float2> ap(npix, make_float2(0.f, 0.f));
+    const double qmax = p->alpha / lambda;
+    long long n_a = 0;
+    for (int sy = 0; sy < ny; ++sy)
+        for (int sx = 0; sx < nx; ++sx) {
+            const double qx = signed_freq(sx, nx) / p->cell[0], qy = signed_freq(sy, ny) / p->cell[1];
+            if (qx * qx + qy * qy <= qmax * qmax) ++n_a;
+        }
+    if (n_a == 0) return PRISM_EINVAL;
+    const double amp = std::sqrt((double)nx * (double)ny) / std::sqrt((double)n_a) / (double)ny;
+    for (int sx = 0; sx < nx; ++sx)
+        for (int sy = 0; sy < ny; ++sy) {
+            const double qx = signed_freq(sx, nx) / p->cell[0], qy = signed_freq(sy, ny) / p->cell[1];
+            const double q2 = qx * qx + qy * qy;
+            if (q2 <= qmax * qmax) {
+                const double chi = aberration(p, lambda, q2);
+                ap[(size_t)sx * ny + sy] = make_float2((float)(amp * std::cos(-chi)), (float)(amp * std::sin(-chi)));
+            }
+        }
+    CU(upload(L.aperture_t, ap, st));
+    std::vector<int> kxs(nx), kys(ny);
+    for (int m = 0; m < nx; ++m) kxs[m] = signed_freq(m, nx);
+    for (int m = 0; m < ny; ++m) kys[m] = signed_freq(m, ny);
+    std::vector<float2> phx, phy;
+    position_phases(p->probes_x, p->probe_origin[0], p->probe_step[0], p->cell[0], kxs, phx);
+    position_phases(p->probes_y, p->probe_origin[1], p->probe_step[1], p->cell[1], kys, phy);
+    CU(upload(L.phase_x, phx, st));
+    CU(upload(L.phase_y, phy, st));
+    std::vector<int> bstart, bpix;
+    ring_lists(p, nx, ny, 1, 1, bstart, bpix);
+    CU(upload(L.bin_start, bstart, st));
+    CU(upload(L.bin_pix, bpix, st));
+    CU(cudaStreamSynchronize(st));
+
+    SliceFeeder& feed = L.feed;
+    feed.v = v; feed.on_host = p->potential_on_host != 0; feed.npix = (int64_t)npix; feed.n_slices = p->n_slices;
+    feed.sigma = sigma; feed.main_stream = st;
+    if ((rc = feed.init())) { feed.release(); return rc; }
+
+    const int n_probes = p->probes_x * p->probes_y;
+    auto run = [&]() -> int {
+        for (int p0 = 0; p0 < n_probes; p0 += L.batch) {
+            const int np = std::min(L.batch, n_probes - p0);
+            ColArgs ca;
+            std::memset(&ca, 0, sizeof(ca));
+            ca.a = L.psi; ca.intensity = L.intensity; ca.tw_y = L.tab.tw_y; ca.prop_x = L.tab.prop_x;
+            ca.prop_y = L.tab.prop_y; ca.ky_lim = L.tab.ky_lim; ca.aperture_t = L.aperture_t;
+            ca.phase_x = L.phase_x; ca.phase_y = L.phase_y; ca.probe0 = p0; ca.probes_x = p->probes_x;
+            ca.n_waves = np; ca.nx = nx; ca.ny = ny;
+            ca.scale = (float)((double)ny / (double)nx);      // I = |Psi_S|^2 / (nx ny), see DESIGN.md
+            RowArgs ra;
+            std::memset(&ra, 0, sizeof(ra));
+            ra.a = L.psi; ra.out = L.psi; ra.t = feed.tbuf; ra.tw_x = L.tab.tw_x; ra.tw_y = L.tab.tw_y;
+            ra.n_waves = np; ra.nx = nx; ra.ny = ny; ra.scale = 1.f;
+            LAUNCH(launch_col_pass(COL_MS_INIT, ca, st));
+            feed.begin_sweep();
+            for (int sl = 0; sl < p->n_slices; ++sl) {
+                int r = feed.get(sl);
+                if (r) return r;
+                LAUNCH(launch_row_pass(ROW_STEP, ra, st));
+                LAUNCH(launch_col_pass(sl == p->n_slices - 1 ? COL_MS_FINAL : COL_STEP, ca, st));
+            }
+            LAUNCH(launch_bin_reduce(L.intensity, (int64_t)npix, L.bin_start, L.bin_pix, nb,
+                                     d_out + (size_t)p0 * nb, np, st));
+        }
+        return PRISM_OK;
+    };
+    rc = run();
+    feed.release();
+    if (rc) return rc;
+    return copy_out(p, out, L.out_stage, out_dev, st);
+}
+
+#pragma GCC visibility pop
+}  // extern "C"

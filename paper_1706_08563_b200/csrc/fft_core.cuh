@@ -1,0 +1,242 @@
+// fft_core.cuh -- register-resident complex64 line FFT for sm_100a.
+//
+// One line of N points is transformed by T = N/E threads holding E points each
+// in registers (thread t holds x[t + T*e], e = 0..E-1, so global loads and stores
+// of a contiguous line are coalesced 8-byte accesses).  The transform is a
+// Stockham autosort FFT in up to three radix stages (N = R1*R2*R3); between
+// stages the threads of the line exchange data through shared memory, whose
+// index space is padded (idx + idx/16) so that both the strided writes and the
+// contiguous reads are bank-conflict free for 8-byte words.  Output is in
+// natural order and lands in the same register layout as the input, so an
+// inverse transform can follow a forward one with no extra exchange.
+//
+// Inter-stage twiddles are exact table values (fp64-built w_N^m, rounded once to
+// fp32) that each thread loads ONCE into registers: they depend on the thread's
+// position in the line, not on the line.
+//
+// The inverse transform is the forward one on (im, re)-swapped data.
+//
+// Implements the transforms of PAPER.md:80 (Eq. 2 needs FFT / inverse FFT around
+// the propagator) and PAPER.md:128 ("the modulus squared of its FFT").
+#pragma once
+#include <cuda_runtime.h>
+
+namespace prism {
+
+__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
+__device__ __forceinline__ float2 cmul(float2 a, float2 b)
+{ return make_float2(fmaf(a.x, b.x, -a.y * b.y), fmaf(a.x, b.y, a.y * b.x)); }
+__device__ __forceinline__ float2 cmul_conj(float2 a, float2 b)   // a * conj(b)
+{ return make_float2(fmaf(a.x, b.x, a.y * b.y), fmaf(a.y, b.x, -a.x * b.y)); }
+__device__ __forceinline__ float2 mul_mi(float2 a) { return make_float2(a.y, -a.x); }   // a * (-i)
+__device__ __forceinline__ float2 cswap(float2 a) { return make_float2(a.y, a.x); }
+
+// ---- forward DFT_R on R registers, natural order in and out ------------------
+template <int R> struct Dft;
+
+template <> struct Dft<1> { __device__ __forceinline__ static void run(float2*) {} };
+
+template <> struct Dft<2> {
+    __device__ __forceinline__ static void run(float2* a)
+    { float2 t = a[0]; a[0] = cadd(t, a[1]); a[1] = csub(t, a[1]); }
+};
+
+template <> struct Dft<4> {
+    __device__ __forceinline__ static void run(float2* a)
+    {
+        float2 t0 = cadd(a[0], a[2]), t1 = csub(a[0], a[2]);
+        float2 t2 = cadd(a[1], a[3]), t3 = mul_mi(csub(a[1], a[3]));
+        a[0] = cadd(t0, t2); a[2] = csub(t0, t2);
+        a[1] = cadd(t1, t3); a[3] = csub(t1, t3);
+    }
+};
+
+template <> struct Dft<8> {
+    __device__ __forceinline__ static void run(float2* a)
+    {
+        const float h = 0.70710678118654752440f;
+        float2 e[4] = { a[0], a[2], a[4], a[6] };
+        float2 o[4] = { a[1], a[3], a[5], a[7] };
+        Dft<4>::run(e); Dft<4>::run(o);
+        // o[k] *= w8^k : w8 = (1-i)/sqrt2, w8^2 = -i, w8^3 = (-1-i)/sqrt2
+        o[1] = make_float2(h * (o[1].x + o[1].y), h * (o[1].y - o[1].x));
+        o[2] = mul_mi(o[2]);
+        o[3] = make_float2(h * (o[3].y - o[3].x), -h * (o[3].x + o[3].y));
+#pragma unroll
+        for (int k = 0; k < 4; ++k) { a[k] = cadd(e[k], o[k]); a[k + 4] = csub(e[k], o[k]); }
+    }
+};
+
+template <> struct Dft<16> {
+    __device__ __forceinline__ static void run(float2* a)
+    {
+        // n = 4 n1 + n2 ; k = k1 + 4 k2.  Y[n2][k1] = DFT4 over n1, then twiddle w16^(n2 k1), DFT4 over n2.
+        const float c1 = 0.92387953251128675613f, s1 = 0.38268343236508977173f;   // cos, sin(pi/8)
+        const float h  = 0.70710678118654752440f;
+        float2 y[4][4];
+#pragma unroll
+        for (int n2 = 0; n2 < 4; ++n2) {
+            y[n2][0] = a[n2]; y[n2][1] = a[n2 + 4]; y[n2][2] = a[n2 + 8]; y[n2][3] = a[n2 + 12];
+            Dft<4>::run(y[n2]);
+        }
+        // w16^m = exp(-2 pi i m / 16): m=1 (c1,-s1) m=2 (h,-h) m=3 (s1,-c1) m=4 (0,-1) m=6 (-h,-h) m=9 (-c1, s1)
+        y[1][1] = cmul(y[1][1], make_float2(c1, -s1));
+        y[1][2] = cmul(y[1][2], make_float2(h, -h));
+        y[1][3] = cmul(y[1][3], make_float2(s1, -c1));
+        y[2][1] = cmul(y[2][1], make_float2(h, -h));
+        y[2][2] = mul_mi(y[2][2]);
+        y[2][3] = cmul(y[2][3], make_float2(-h, -h));
+        y[3][1] = cmul(y[3][1], make_float2(s1, -c1));
+        y[3][2] = cmul(y[3][2], make_float2(-h, -h));
+        y[3][3] = cmul(y[3][3], make_float2(-c1, s1));
+#pragma unroll
+        for (int k1 = 0; k1 < 4; ++k1) {
+            float2 z[4] = { y[0][k1], y[1][k1], y[2][k1], y[3][k1] };
+            Dft<4>::run(z);
+            a[k1] = z[0]; a[k1 + 4] = z[1]; a[k1 + 8] = z[2]; a[k1 + 12] = z[3];
+        }
+    }
+};
+
+// ---- plan ---------------------------------------------------------------------
+template <int N_, int E_, int R1_, int R2_, int R3_>
+struct Plan {
+    static constexpr int N = N_, E = E_, T = N_ / E_, R1 = R1_, R2 = R2_, R3 = R3_;
+    static_assert(R1_ * R2_ * R3_ == N_, "radices must multiply to N");
+    static_assert(E_ % R1_ == 0 && E_ % R2_ == 0 && E_ % R3_ == 0, "each radix must divide E");
+    static constexpr int NB1 = E_ / R1_, NB2 = E_ / R2_, NB3 = (R3_ > 1 ? E_ / R3_ : 1);
+    // stage-2 twiddles depend on (t + T m) mod R1: shared by all m when R1 divides T
+    static constexpr bool S2_SHARED = (T % R1_ == 0);
+    static constexpr int  S2_SETS = S2_SHARED ? 1 : NB2;
+    static constexpr int  PADDED = N_ + N_ / 16;      // padded exchange index space
+};
+
+template <int N> struct PlanFor;
+template <> struct PlanFor<16>   { using type = Plan<16, 4, 4, 4, 1>; };
+template <> struct PlanFor<32>   { using type = Plan<32, 8, 8, 4, 1>; };
+template <> struct PlanFor<64>   { using type = Plan<64, 8, 8, 8, 1>; };
+template <> struct PlanFor<128>  { using type = Plan<128, 16, 16, 8, 1>; };
+template <> struct PlanFor<256>  { using type = Plan<256, 16, 16, 16, 1>; };
+template <> struct PlanFor<512>  { using type = Plan<512, 16, 16, 16, 2>; };
+template <> struct PlanFor<1024> { using type = Plan<1024, 16, 16, 16, 4>; };
+template <> struct PlanFor<2048> { using type = Plan<2048, 16, 16, 16, 8>; };
+
+__device__ __forceinline__ int pad16(int i) { return i + (i >> 4); }
+
+// Per-thread twiddles, loaded once from the table tw[m] = exp(-2 pi i m / N).
+template <class P>
+struct Twiddles {
+    float2 s2[P::S2_SETS][P::R2 > 1 ? P::R2 - 1 : 1];
+    float2 s3[P::NB3][P::R3 > 1 ? P::R3 - 1 : 1];
+
+    __device__ __forceinline__ void load(const float2* __restrict__ tw, int t)
+    {
+#pragma unroll
+        for (int m = 0; m < P::S2_SETS; ++m) {
+            int k = (t + P::T * m) % P::R1;
+#pragma unroll
+            for (int r = 1; r < P::R2; ++r)
+                s2[m][r - 1] = __ldg(tw + ((r * k * (P::N / (P::R1 * P::R2))) & (P::N - 1)));
+        }
+        if (P::R3 > 1) {
+#pragma unroll
+            for (int m = 0; m < P::NB3; ++m) {
+                int k = (t + P::T * m) % (P::R1 * P::R2);
+#pragma unroll
+                for (int r = 1; r < P::R3; ++r)
+                    s3[m][r - 1] = __ldg(tw + ((r * k) & (P::N - 1)));
+            }
+        }
+    }
+};
+
+// Shared-memory view of one line's exchange space: element idx lives at
+// base[pad16(idx) * stride].  stride = 1 for a row buffer, (W+1) for a column of
+// a padded [rows][W+1] tile.
+struct LineSmem {
+    float2* base;
+    int stride;
+    __device__ __forceinline__ void  st(int idx, float2 v) const { base[pad16(idx) * stride] = v; }
+    __device__ __forceinline__ float2 ld(int idx) const { return base[pad16(idx) * stride]; }
+};
+
+// barrier among the threads of one line (or more): whole warp if the line fits in
+// one, else the whole CTA (every thread of the CTA runs the same sequence).
+template <class P>
+__device__ __forceinline__ void line_sync()
+{
+    if (P::T <= 32) __syncwarp(); else __syncthreads();
+}
+
+// Forward transform of the line held as v[e] = x[t + T e].  Begins with a
+// line_sync(), so `sm` may alias storage the line's threads have just read.
+template <class P>
+__device__ __forceinline__ void fft_forward(float2 (&v)[P::E], const Twiddles<P>& tw, int t, const LineSmem& sm)
+{
+    constexpr int E = P::E, T = P::T;
+    line_sync<P>();                          // earlier readers of `sm` (previous transform, tile loads) are done
+    // ---- stage 1: radix R1, Ns = 1, no twiddles ----
+#pragma unroll
+    for (int m = 0; m < P::NB1; ++m) {
+        float2 a[P::R1];
+#pragma unroll
+        for (int r = 0; r < P::R1; ++r) a[r] = v[m + P::NB1 * r];
+        Dft<P::R1>::run(a);
+        const int j = t + T * m;
+#pragma unroll
+        for (int r = 0; r < P::R1; ++r) sm.st(j * P::R1 + r, a[r]);
+    }
+    line_sync<P>();
+#pragma unroll
+    for (int e = 0; e < E; ++e) v[e] = sm.ld(t + T * e);
+    // ---- stage 2: radix R2, Ns = R1 ----
+    if (P::R3 > 1) line_sync<P>();           // all reads done before the next exchange overwrites
+#pragma unroll
+    for (int m = 0; m < P::NB2; ++m) {
+        float2 a[P::R2];
+        a[0] = v[m];
+#pragma unroll
+        for (int r = 1; r < P::R2; ++r) a[r] = cmul(v[m + P::NB2 * r], tw.s2[P::S2_SHARED ? 0 : m][r - 1]);
+        Dft<P::R2>::run(a);
+        if (P::R3 == 1) {
+#pragma unroll
+            for (int r = 0; r < P::R2; ++r) v[m + P::NB2 * r] = a[r];
+        } else {
+            const int j = t + T * m;
+            const int k = j % P::R1;
+            const int idx = (j / P::R1) * (P::R1 * P::R2) + k;
+#pragma unroll
+            for (int r = 0; r < P::R2; ++r) sm.st(idx + r * P::R1, a[r]);
+        }
+    }
+    if (P::R3 > 1) {
+        line_sync<P>();
+#pragma unroll
+        for (int e = 0; e < E; ++e) v[e] = sm.ld(t + T * e);
+        // ---- stage 3: radix R3, Ns = R1 R2, in place ----
+#pragma unroll
+        for (int m = 0; m < P::NB3; ++m) {
+            float2 a[P::R3 > 1 ? P::R3 : 1];
+            a[0] = v[m];
+#pragma unroll
+            for (int r = 1; r < P::R3; ++r) a[r] = cmul(v[m + P::NB3 * r], tw.s3[m][r - 1]);
+            Dft<P::R3>::run(a);
+#pragma unroll
+            for (int r = 0; r < P::R3; ++r) v[m + P::NB3 * r] = a[r];
+        }
+    }
+}
+
+// Unscaled inverse transform: forward transform of the (im, re)-swapped data.
+template <class P>
+__device__ __forceinline__ void fft_inverse(float2 (&v)[P::E], const Twiddles<P>& tw, int t, const LineSmem& sm)
+{
+#pragma unroll
+    for (int e = 0; e < P::E; ++e) v[e] = cswap(v[e]);
+    fft_forward<P>(v, tw, t, sm);
+#pragma unroll
+    for (int e = 0; e < P::E; ++e) v[e] = cswap(v[e]);
+}
+
+}  // namespace prism

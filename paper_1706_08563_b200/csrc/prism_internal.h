@@ -1,0 +1,91 @@
+// prism_internal.h -- declarations shared by the translation units of
+// libprism_b200.so (not part of the public C ABI, see include/prism.h).
+#pragma once
+#include <cuda_runtime.h>
+#include <stddef.h>
+#include <stdint.h>
+
+namespace prism {
+
+// ---- slice-step passes (slice_pass.cu) -----------------------------------------
+// Waves live in "mixed space" A[w][y][kx] = sum_x psi[w][y][x] exp(-2 pi i kx x / nx)
+// between the two passes of a slice.
+enum RowMode {
+    ROW_INIT  = 0,   // plane wave b  -> * t            -> FFT_x -> A          (first slice, no read)
+    ROW_STEP  = 1,   // A -> IFFT_x   -> * t            -> FFT_x -> A
+    ROW_FINAL = 2,   // A -> IFFT_x   -> * scale        -> out   (real-space exit wave, S-matrix layer)
+    ROW_FFT   = 3,   // a -> FFT_x -> a                           (probe windows, stage 2)
+};
+struct RowArgs {
+    float2*       a;          // [n_waves][ny][nx] in/out
+    float2*       out;        // ROW_FINAL destination (may alias a)
+    const float2* t;          // [ny][nx] transmission function of this slice (ROW_INIT, ROW_STEP)
+    const float2* tw_x;       // exp(-2 pi i m / nx), m < nx
+    const float2* tw_y;       // exp(-2 pi i m / ny), m < ny   (ROW_INIT phase of the plane wave)
+    const int2*   beams;      // [n_waves] (kx, ky)             (ROW_INIT)
+    int           n_waves, nx, ny;
+    float         scale;      // ROW_INIT: plane-wave amplitude; ROW_FINAL: output scale
+};
+cudaError_t launch_row_pass(RowMode mode, const RowArgs& args, cudaStream_t stream);
+
+enum ColMode {
+    COL_STEP     = 0,   // A -> FFT_y -> * P -> IFFT_y -> A
+    COL_MS_INIT  = 1,   // probe spectrum Psi0(kx, ky) -> IFFT_y -> A          (multislice start, no read)
+    COL_MS_FINAL = 2,   // A -> FFT_y -> * P -> |.|^2 -> intensity[w][kx][ky]  (multislice end, no IFFT)
+    COL_ABS2     = 3,   // a -> FFT_y -> |.|^2 * scale -> intensity[w][kx][ky] (probe windows, stage 2)
+};
+struct ColArgs {
+    float2*       a;          // [n_waves][ny][nx] in/out
+    float*        intensity;  // [n_waves][nx][ny]  (COL_MS_FINAL, COL_ABS2) -- transposed: ky contiguous
+    const float2* tw_y;       // exp(-2 pi i m / ny)
+    const float2* prop_x;     // [nx] x-factor of the propagator (all scale factors folded in)
+    const float2* prop_y;     // [ny] y-factor
+    const int*    ky_lim;     // [nx] band-limit: |ky| <= ky_lim[kx] passes, -1 = whole column masked
+    // COL_MS_INIT
+    const float2* aperture_t; // [nx][ny] A_k exp(-i chi_k) * amplitude (transposed, ky contiguous)
+    const float2* phase_x;    // [probes_x][nx] exp(-2 pi i kx x_p / lx)
+    const float2* phase_y;    // [probes_y][ny] exp(-2 pi i ky y_p / ly)
+    int           probe0, probes_x;   // wave w is probe probe0 + w; (px, py) = (p % probes_x, p / probes_x)
+    int           n_waves, nx, ny;
+    float         scale;      // COL_ABS2 / COL_MS_FINAL intensity scale
+};
+cudaError_t launch_col_pass(ColMode mode, const ColArgs& args, cudaStream_t stream);
+
+// t = exp(i sigma V) for one slice (Eq. 1), fp64 sincos rounded once to fp32
+cudaError_t launch_transmission(const float* v, float2* t, double sigma, int64_t npix, cudaStream_t stream);
+
+// ---- stage 2 (output.cu) ---------------------------------------------------------
+struct BeamSumArgs {
+    const float2* s;          // [n_beams][ny][nx] compact S-matrix
+    float2*       w;          // [n_probes_batch][my][mx] summed windows (out)
+    const float2* coef_b;     // [n_beams]  A_b exp(-i chi_b) * scale
+    const float2* phase_x;    // [probes_x][n_beams] exp(-2 pi i kx_b x_p / lx)
+    const float2* phase_y;    // [probes_y][n_beams] exp(-2 pi i ky_b y_p / ly)
+    const int*    win_x0;     // [probes_x] first window column (already wrapped into [0, nx))
+    const int*    win_y0;     // [probes_y] first window row
+    int           n_beams, nx, ny, mx, my;
+    int           probe0, n_probes_batch, probes_x;
+};
+cudaError_t launch_beam_sum(const BeamSumArgs& args, cudaStream_t stream);
+
+// out[w][bin] = sum of intensity[w][pix] over the pixels listed for the bin (CSR), fixed order
+cudaError_t launch_bin_reduce(const float* intensity, int64_t npix, const int* bin_start,
+                              const int* bin_pix, int n_bins, float* out, int n_waves,
+                              cudaStream_t stream);
+
+// ---- potential (potential.cu) ------------------------------------------------------
+struct PotAtom { double x, y; int32_t lut; int32_t pad; };
+struct PotentialArgs {
+    const PotAtom* atoms;       // sorted by (slice, tile_y, tile_x)
+    const int*     cell_start;  // [n_slices * tiles_y * tiles_x + 1]
+    const float*   lut_v;       // [n_luts][lut_n]
+    const double*  lut_rcut;    // [n_luts]
+    int            lut_n;
+    int            nx, ny, tiles_x, tiles_y, tile, reach_tiles;
+    double         px, py, lx, ly;
+    int            slice0, n_slices_chunk;   // slices [slice0, slice0 + n_slices_chunk) -> v_out
+    float*         v_out;       // [n_slices_chunk][ny][nx]
+};
+cudaError_t launch_potential(const PotentialArgs& args, cudaStream_t stream);
+
+}  // namespace prism

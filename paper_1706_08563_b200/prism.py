@@ -1,0 +1,184 @@
+"""Thin ctypes binding of ``libprism_b200.so`` (C ABI: ``include/prism.h``).
+
+Argument marshalling only -- every step of the path runs in the CUDA kernels of
+``csrc/``.  PyTorch supplies device memory and the current CUDA stream; nothing
+here computes.  There is no CPU fallback: if the library is missing, importing
+this module raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libprism_b200.so")
+
+PRISM_OK, PRISM_EINVAL, PRISM_ENOMEM, PRISM_ECUDA, PRISM_EUNSUPPORTED, PRISM_ENOLUT = 0, -1, -2, -3, -4, -5
+WS_SMATRIX, WS_OUTPUT, WS_MULTISLICE, WS_POTENTIAL = 0, 1, 2, 3
+
+EXPORTS = ["prism_workspace_bytes", "prism_num_bins", "prism_num_beams", "prism_constants",
+           "prism_build_potential", "prism_compute_smatrix", "prism_compute_output",
+           "multislice_compute_output", "prism_strerror", "prism_last_error", "prism_launch_count"]
+
+
+class Params(C.Structure):
+    """``prism_params`` of include/prism.h (same field order and types)."""
+    _fields_ = [
+        ("cell", C.c_double * 3), ("nx", C.c_int32), ("ny", C.c_int32),
+        ("slice_thickness", C.c_double), ("n_slices", C.c_int32),
+        ("voltage", C.c_double), ("alpha", C.c_double), ("defocus", C.c_double), ("cs", C.c_double),
+        ("f", C.c_int32), ("probes_x", C.c_int32), ("probes_y", C.c_int32),
+        ("probe_origin", C.c_double * 2), ("probe_step", C.c_double * 2),
+        ("det_step", C.c_double), ("det_max", C.c_double),
+        ("batch", C.c_int32), ("potential_on_host", C.c_int32),
+    ]
+
+
+class Lut(C.Structure):
+    _fields_ = [("z", C.c_int32), ("n", C.c_int32), ("r_cut", C.c_double), ("v", C.POINTER(C.c_float))]
+
+
+class PrismError(RuntimeError):
+    def __init__(self, code: int, where: str):
+        self.code = code
+        msg = _lib.prism_strerror(code).decode()
+        detail = _lib.prism_last_error().decode() if code == PRISM_ECUDA else ""
+        super().__init__(f"{where}: {msg} ({code}) {detail}".strip())
+
+
+def _load() -> C.CDLL:
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(
+            f"{LIB_PATH} is not built: run `python -m paper_1706_08563_b200.build` "
+            "(nvcc, sm_100a).  There is no CPU fallback.")
+    lib = C.CDLL(LIB_PATH)
+    vp, i32, i64, sz = C.c_void_p, C.c_int32, C.c_int64, C.c_size_t
+    pp = C.POINTER(Params)
+    lib.prism_workspace_bytes.restype = sz
+    lib.prism_workspace_bytes.argtypes = [pp, i32]
+    lib.prism_num_bins.restype = i32
+    lib.prism_num_bins.argtypes = [pp]
+    lib.prism_num_beams.restype = C.c_int
+    lib.prism_num_beams.argtypes = [pp, C.POINTER(i32)]
+    lib.prism_constants.restype = C.c_int
+    lib.prism_constants.argtypes = [C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+    lib.prism_build_potential.restype = C.c_int
+    lib.prism_build_potential.argtypes = [pp, vp, vp, i64, C.POINTER(Lut), i32, vp, vp, sz, vp]
+    lib.prism_compute_smatrix.restype = C.c_int
+    lib.prism_compute_smatrix.argtypes = [pp, vp, vp, vp, vp, sz, vp]
+    lib.prism_compute_output.restype = C.c_int
+    lib.prism_compute_output.argtypes = [pp, vp, vp, i32, vp, vp, sz, vp]
+    lib.multislice_compute_output.restype = C.c_int
+    lib.multislice_compute_output.argtypes = [pp, vp, vp, vp, sz, vp]
+    lib.prism_strerror.restype = C.c_char_p
+    lib.prism_strerror.argtypes = [C.c_int]
+    lib.prism_last_error.restype = C.c_char_p
+    lib.prism_launch_count.restype = i64
+    lib.prism_launch_count.argtypes = [i32]
+    return lib
+
+
+_lib = _load()
+
+
+def _check(code: int, where: str):
+    if code != PRISM_OK:
+        raise PrismError(code, where)
+
+
+def params_from_workload(w, **override) -> Params:
+    """Fill ``prism_params`` from a ``workloads.Workload`` (plain field copy)."""
+    p = Params()
+    p.cell[:] = w.cell
+    p.nx, p.ny = w.nx, w.ny
+    p.slice_thickness, p.n_slices = w.dz, w.n_slices
+    p.voltage, p.alpha, p.defocus, p.cs = w.voltage, w.alpha, w.defocus, w.cs
+    p.f, p.probes_x, p.probes_y = w.f, w.probes_x, w.probes_y
+    p.probe_origin[:] = w.probe_origin
+    p.probe_step[:] = w.probe_step
+    p.det_step, p.det_max = w.det_step, w.det_max
+    p.batch, p.potential_on_host = w.batch, w.potential_on_host
+    for k, v in override.items():
+        setattr(p, k, v)
+    return p
+
+
+def _stream_ptr(stream=None) -> int:
+    import torch
+    s = torch.cuda.current_stream() if stream is None else stream
+    return int(s.cuda_stream)
+
+
+def _ptr(t) -> int:
+    return int(t.data_ptr())
+
+
+def workspace_bytes(p: Params, which: int, n_atoms: int = 0) -> int:
+    n = int(_lib.prism_workspace_bytes(C.byref(p), which))
+    if n == 0:
+        raise PrismError(PRISM_EINVAL, "prism_workspace_bytes")
+    return n + (32 * n_atoms + 256 if which == WS_POTENTIAL else 0)
+
+
+def num_bins(p: Params) -> int:
+    return int(_lib.prism_num_bins(C.byref(p)))
+
+
+def num_beams(p: Params) -> int:
+    n = C.c_int32(0)
+    _check(_lib.prism_num_beams(C.byref(p), C.byref(n)), "prism_num_beams")
+    return n.value
+
+
+def constants(voltage: float):
+    lam, sig = C.c_double(), C.c_double()
+    _check(_lib.prism_constants(voltage, C.byref(lam), C.byref(sig)), "prism_constants")
+    return lam.value, sig.value
+
+
+def launch_count(reset: bool = False) -> int:
+    return int(_lib.prism_launch_count(1 if reset else 0))
+
+
+def build_potential(p: Params, atoms_xyz, z_number, lut_z, r_cut, lut_v, v_out, workspace, stream=None):
+    """``prism_build_potential``.  atoms/z/luts are host numpy arrays; ``v_out`` is a CUDA tensor
+    ``[n_slices][ny][nx]`` fp32, or a pinned host tensor when ``p.potential_on_host``."""
+    atoms = np.ascontiguousarray(atoms_xyz, dtype=np.float64).reshape(-1, 3)
+    zn = np.ascontiguousarray(z_number, dtype=np.int32)
+    tabs = np.ascontiguousarray(lut_v, dtype=np.float32).reshape(len(lut_z), -1)
+    luts = (Lut * len(lut_z))()
+    for i, z in enumerate(lut_z):
+        luts[i].z, luts[i].n, luts[i].r_cut = int(z), tabs.shape[1], float(r_cut)
+        luts[i].v = tabs[i].ctypes.data_as(C.POINTER(C.c_float))
+    _check(_lib.prism_build_potential(C.byref(p), atoms.ctypes.data, zn.ctypes.data, len(zn), luts, len(lut_z),
+                                      _ptr(v_out), _ptr(workspace), workspace.numel() * workspace.element_size(),
+                                      _stream_ptr(stream)), "prism_build_potential")
+    return v_out
+
+
+def compute_smatrix(p: Params, v, s_out, workspace, stream=None):
+    """``prism_compute_smatrix``.  Returns the host beam list ``[n_beams][2]`` int32."""
+    beams = np.empty((num_beams(p), 2), dtype=np.int32)
+    _check(_lib.prism_compute_smatrix(C.byref(p), _ptr(v), beams.ctypes.data, _ptr(s_out), _ptr(workspace),
+                                      workspace.numel() * workspace.element_size(), _stream_ptr(stream)),
+           "prism_compute_smatrix")
+    return beams
+
+
+def compute_output(p: Params, s, beams, out, workspace, stream=None):
+    """``prism_compute_output``.  ``out`` fp32 ``[probes_y][probes_x][n_bins]``, CUDA or (pinned) host tensor."""
+    beams = np.ascontiguousarray(beams, dtype=np.int32).reshape(-1, 2)
+    _check(_lib.prism_compute_output(C.byref(p), _ptr(s), beams.ctypes.data, len(beams), _ptr(out), _ptr(workspace),
+                                     workspace.numel() * workspace.element_size(), _stream_ptr(stream)),
+           "prism_compute_output")
+    return out
+
+
+def multislice_output(p: Params, v, out, workspace, stream=None):
+    """``multislice_compute_output``."""
+    _check(_lib.multislice_compute_output(C.byref(p), _ptr(v), _ptr(out), _ptr(workspace),
+                                          workspace.numel() * workspace.element_size(), _stream_ptr(stream)),
+           "multislice_compute_output")
+    return out

@@ -1,0 +1,189 @@
+"""Parity of the CUDA path (through the C ABI) with the fp64 oracle, element by element on
+the same seeded inputs.  Tolerances: BASELINE.json north_star -- detector-ring intensities
+within relative L2 1e-4 (1e-3 for 2048^2 with >= 400 slices); DESIGN.md derives the
+per-stage bounds used for the potential (1e-6) and the S-matrix layers (2e-5)."""
+import numpy as np
+import pytest
+
+import oracle as O
+from helpers import oracle_params, oracle_potential, rel_l2
+from paper_1706_08563_b200 import workloads as W
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+TOL_OUT = 1e-4
+TOL_V = 1e-6
+TOL_S = 2e-5
+
+
+@pytest.fixture(scope="module")
+def G():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import gpu_helpers
+    return gpu_helpers
+
+
+def _cases():
+    return {
+        "PR1": W.pr1(),
+        # 128^2, f=2 -> 64^2 windows; off-pixel probe positions; defocus + Cs
+        "T128f2": W.scaled_test_case(128, 6, 2, 5, alpha_mrad=25.0, defocus=40.0, cs=2.0e4,
+                                     probe_offset=(0.137, 0.291), seed_index=1),
+        # 128^2, f=4 -> 32^2 windows, 300 kV, heavy atoms
+        "T128f4": W.scaled_test_case(128, 5, 4, 6, voltage=300e3, alpha_mrad=20.0, z_choices=(79, 33),
+                                     seed_index=2),
+        # 256^2, f=2 -> 128^2 windows (the window size of configs 3-5)
+        "T256f2": W.scaled_test_case(256, 4, 2, 3, voltage=300e3, alpha_mrad=20.0, seed_index=3,
+                                     probe_offset=(0.05, 0.0)),
+        # 512^2: three-stage FFT plan, f=8 -> 64^2 windows
+        "T512f8": W.scaled_test_case(512, 3, 8, 3, voltage=300e3, alpha_mrad=20.0, seed_index=4, density=0.02),
+    }
+
+
+CASES = _cases()
+
+
+@pytest.mark.parametrize("name", list(CASES))
+def test_potential_parity(G, name):
+    w = CASES[name]
+    v = G.gpu_potential(w).cpu().numpy().astype(np.float64)
+    ref = oracle_potential(w)
+    assert v.shape == ref.shape
+    assert rel_l2(v, ref) < TOL_V
+    assert np.array_equal(v == 0, ref == 0) or np.count_nonzero((v == 0) != (ref == 0)) <= 2
+
+
+@pytest.mark.parametrize("name", list(CASES))
+def test_smatrix_parity(G, name):
+    w = CASES[name]
+    p = oracle_params(w)
+    v = G.gpu_potential(w)
+    s, beams = G.gpu_smatrix(w, v)
+    ref_beams = O.beams(p)
+    assert set(map(tuple, beams.tolist())) == set(map(tuple, ref_beams.tolist()))
+    v_ref = oracle_potential(w)
+    pick = np.unique(np.linspace(0, len(beams) - 1, 7).astype(int)) if name != "PR1" else np.arange(len(beams))
+    s_host = s.cpu().numpy()
+    for b in pick:
+        ref = O.smatrix_layer(p, v_ref, int(beams[b, 0]), int(beams[b, 1]))
+        assert rel_l2(s_host[b].astype(np.complex128), ref) < TOL_S, (name, b)
+
+
+@pytest.mark.parametrize("name", list(CASES))
+def test_prism_output_parity(G, name):
+    w = CASES[name]
+    p = oracle_params(w)
+    v = G.gpu_potential(w)
+    s, beams = G.gpu_smatrix(w, v)
+    out = G.gpu_prism_output(w, s, beams)
+    v_ref = oracle_potential(w)
+    s_ref = O.smatrix(p, v_ref, beams)
+    ref = O.prism_probes(p, s_ref, beams, w.probe_xy())
+    assert out.shape == ref.shape
+    assert rel_l2(out, ref) < TOL_OUT
+    d = G.dark_field(w, p)
+    assert ref[:, d:].sum() > 0
+    assert rel_l2(out[:, d:], ref[:, d:]) < 5 * TOL_OUT        # dark field alone (reading R22)
+
+
+@pytest.mark.parametrize("name", ["PR1", "T128f2", "T256f2", "T512f8"])
+def test_multislice_parity(G, name):
+    w = CASES[name]
+    p = oracle_params(w)
+    v = G.gpu_potential(w)
+    out = G.gpu_multislice(w, v)
+    ref = O.multislice_probes(p, oracle_potential(w), w.probe_xy())
+    assert rel_l2(out, ref) < TOL_OUT
+    d = G.dark_field(w, p)
+    assert rel_l2(out[:, d:], ref[:, d:]) < 5 * TOL_OUT
+
+
+def test_prism_f1_equals_multislice_on_gpu(G):
+    w = CASES["PR1"]
+    v = G.gpu_potential(w)
+    s, beams = G.gpu_smatrix(w, v)
+    assert rel_l2(G.gpu_prism_output(w, s, beams), G.gpu_multislice(w, v)) < TOL_OUT
+
+
+def test_results_do_not_depend_on_batch_or_memory_mode(G):
+    from paper_1706_08563_b200 import prism
+    w = CASES["T128f2"]
+    v = G.gpu_potential(w)
+    v_host = G.gpu_potential(w, on_host=True)
+    assert torch.equal(v.cpu(), v_host)                              # same kernel, staged copy
+    s0, beams = G.gpu_smatrix(w, v)
+    for kw in [dict(batch=1), dict(batch=5), dict(batch=0)]:
+        p = prism.params_from_workload(w, **kw)
+        s1, b1 = G.gpu_smatrix(w, v, p)
+        assert np.array_equal(beams, b1) and torch.equal(s0, s1)
+    s2, _ = G.gpu_smatrix(w, v_host)                                  # streamed from pinned host memory
+    assert torch.equal(s0, s2)
+    s3, _ = G.gpu_smatrix(w, v_host, prism.params_from_workload(w, batch=7))
+    assert torch.equal(s0, s3)
+    out0 = G.gpu_prism_output(w, s0, beams)
+    for b in [1, 4, 25]:
+        assert np.array_equal(out0, G.gpu_prism_output(w, s0, beams, prism.params_from_workload(w, batch=b)))
+    assert np.array_equal(out0, G.gpu_prism_output(w, s0, beams, host_out=True))
+    m0 = G.gpu_multislice(w, v)
+    for b in [1, 3]:
+        assert np.array_equal(m0, G.gpu_multislice(w, v, prism.params_from_workload(w, batch=b)))
+    assert np.array_equal(m0, G.gpu_multislice(w, v_host, prism.params_from_workload(w, batch=4)))
+    assert np.array_equal(m0, G.gpu_multislice(w, v, host_out=True))
+
+
+def test_empty_specimen_closed_form(G):
+    w = CASES["T128f4"]
+    w0 = w.with_(atoms=np.zeros((0, 3)), z=np.zeros(0, np.int32))
+    p = oracle_params(w0)
+    from paper_1706_08563_b200 import prism
+    pp = prism.params_from_workload(w0)
+    v = torch.zeros((w0.n_slices, w0.ny, w0.nx), dtype=torch.float32, device=G.DEV)
+    s, beams = G.gpu_smatrix(w0, v, pp)
+    out = G.gpu_prism_output(w0, s, beams, pp)
+    lam, _ = O.constants(w0.voltage)
+    ang = lam * np.hypot(beams[:, 0] / w0.cell[0], beams[:, 1] / w0.cell[1])
+    want = np.bincount(np.floor(ang / w0.det_step).astype(int), minlength=out.shape[1])[:out.shape[1]] / len(beams)
+    assert np.max(np.abs(out - want[None, :])) < 2e-6
+    ms = G.gpu_multislice(w0, v, pp)
+    ref = O.multislice_probes(p, np.zeros((w0.n_slices, w0.ny, w0.nx)), w0.probe_xy()[:1])
+    assert np.max(np.abs(ms - ref)) < 2e-6
+    # a potential builder call with zero atoms writes zeros
+    assert torch.count_nonzero(G.gpu_potential(w0)) == 0
+
+
+def test_single_slice_and_rectangular_probe_grid(G):
+    w = W.scaled_test_case(64, 1, 2, 4, seed_index=5, density=0.2).with_(probes_x=3, probes_y=5,
+                                                                       probe_step=(1.3, 0.7))
+    p = oracle_params(w)
+    v = G.gpu_potential(w)
+    s, beams = G.gpu_smatrix(w, v)
+    out = G.gpu_prism_output(w, s, beams)
+    v_ref = oracle_potential(w)
+    ref = O.prism_probes(p, O.smatrix(p, v_ref, beams), beams, w.probe_xy())
+    assert out.shape == (15, O.num_bins(p)) and rel_l2(out, ref) < TOL_OUT
+    assert rel_l2(G.gpu_multislice(w, v), O.multislice_probes(p, v_ref, w.probe_xy())) < TOL_OUT
+
+
+def test_error_codes(G):
+    from paper_1706_08563_b200 import prism
+    w = CASES["PR1"]
+    p = prism.params_from_workload(w)
+    v = torch.zeros((w.n_slices, w.ny, w.nx), dtype=torch.float32, device=G.DEV)
+    s = torch.empty((prism.num_beams(p), w.ny, w.nx), dtype=torch.complex64, device=G.DEV)
+    tiny = torch.empty(1024, dtype=torch.uint8, device=G.DEV)
+    with pytest.raises(prism.PrismError) as e:
+        prism.compute_smatrix(p, v, s, tiny)
+    assert e.value.code == prism.PRISM_ENOMEM
+    bad = prism.params_from_workload(w, nx=96)
+    with pytest.raises(prism.PrismError) as e:
+        prism.num_beams(bad)
+    assert e.value.code == prism.PRISM_EINVAL
+    bad = prism.params_from_workload(w, alpha=0.09)                   # beyond the 2/3 band-limit (83.6 mrad)
+    with pytest.raises(prism.PrismError):
+        prism.num_beams(bad)
+    lut_z, r_cut, lut_v = w.lut()
+    with pytest.raises(prism.PrismError) as e:
+        prism.build_potential(p, [[1.0, 1.0, 1.0]], [13], lut_z, r_cut, lut_v, v, G.ws(p, prism.WS_POTENTIAL, 1))
+    assert e.value.code == prism.PRISM_ENOLUT
