@@ -147,7 +147,7 @@ def build_potential(p: Params, atoms_xyz, z_number, lut_z, r_cut, lut_v, v_out, 
     ``[n_slices][ny][nx]`` fp32, or a pinned host tensor when ``p.potential_on_host``."""
     atoms = np.ascontiguousarray(atoms_xyz, dtype=np.float64).reshape(-1, 3)
     zn = np.ascontiguousarray(z_number, dtype=np.int32)
-    tabs = np.ascontiguousarray(lut_v, dtype=np.float32).reshape(len(lut_z), -1)
+    tabs = np.ascontiguousarray(lut_v, dtype=np.float32).reshape(len(lut_z), -1 if len(lut_z) else 0)
     luts = (Lut * len(lut_z))()
     for i, z in enumerate(lut_z):
         luts[i].z, luts[i].n, luts[i].r_cut = int(z), tabs.shape[1], float(r_cut)
