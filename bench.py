@@ -1,0 +1,354 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line for the PRISM hot path on N B200s (contract: task prompt / DESIGN.md).
+
+A step = one pass of the whole hot path for one frozen-phonon configuration of the workload:
+prism_build_potential -> prism_compute_smatrix -> prism_compute_output (all section 8(a) rows).
+`value` = PRISM probes/s over the whole job (all ranks), device-timed with CUDA events on the
+launching stream; `beam_slices_per_s` is reported beside it (BASELINE.json names both).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload P8|P4|P16|PR1] [--impl reference]
+
+N > 1 (torchrun): frozen-phonon configurations are independent problems, so rank r
+takes configurations r, r+N, ... with no collective on the data path ("weak" scaling); the only
+exchange is one NCCL all-reduce of the [probes][rings] sums for the phonon average.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+METRIC = "prism_probes_per_s"
+UNIT = "probes/s"
+FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12      # 148 SMs x 128 FMA lanes x 2 x 1.965 GHz
+WORKLOAD_NOTE = {
+    "PR1": "BASELINE.json configs[0]", "MS2": "BASELINE.json configs[1]", "P4": "BASELINE.json configs[2]",
+    "P8": "BASELINE.json configs[3]", "P16": "BASELINE.json configs[4]",
+}
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as fh:
+            d = json.load(fh)
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+# ------------------------------------------------------------------------------------------------ clocks
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index: int):
+        super().__init__(daemon=True)
+        self.index, self.samples, self.reasons, self.max_mhz = index, [], set(), None
+        self._stop_evt = threading.Event()
+
+    def run(self):
+        try:
+            import pynvml as nv
+            nv.nvmlInit()
+            h = nv.nvmlDeviceGetHandleByIndex(self.index)
+            self.max_mhz = nv.nvmlDeviceGetMaxClockInfo(h, nv.NVML_CLOCK_SM)
+            names = {
+                getattr(nv, "nvmlClocksThrottleReasonHwSlowdown", 0x8): "hw_slowdown",
+                getattr(nv, "nvmlClocksThrottleReasonHwThermalSlowdown", 0x40): "hw_thermal_slowdown",
+                getattr(nv, "nvmlClocksThrottleReasonSwThermalSlowdown", 0x20): "sw_thermal_slowdown",
+                getattr(nv, "nvmlClocksThrottleReasonSwPowerCap", 0x4): "sw_power_cap",
+                getattr(nv, "nvmlClocksThrottleReasonHwPowerBrakeSlowdown", 0x80): "hw_power_brake",
+            }
+            while not self._stop_evt.is_set():
+                self.samples.append(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM))
+                mask = nv.nvmlDeviceGetCurrentClocksThrottleReasons(h)
+                for bit, name in names.items():
+                    if mask & bit:
+                        self.reasons.add(name)
+                time.sleep(0.1)
+        except Exception as exc:  # NVML unavailable: report that rather than invent numbers
+            self.reasons.add(f"nvml_unavailable:{type(exc).__name__}")
+
+    def stop(self):
+        self._stop_evt.set()
+        self.join(timeout=2)
+        return {"sm_mhz": statistics.median(self.samples) if self.samples else None,
+                "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+# ------------------------------------------------------------------------------------------------ oracle arm
+def oracle_params(O, w):
+    return O.Params(w.cell[0], w.cell[1], w.cell[2], w.nx, w.ny, w.n_slices, w.dz, w.voltage, w.alpha,
+                    w.defocus, w.cs, w.f, w.det_step, w.det_max)
+
+
+def oracle_sample(w, budget_s: float = 20.0):
+    """Time the oracle, as it stands, on a bounded sample of the workload and extrapolate linearly in
+    beams and probes (the paper's own practice).  Returns (probes/s, description, dict)."""
+    import oracle as O
+    from paper_1706_08563_b200 import workloads  # noqa: F401  (inputs only)
+    cores = O.num_threads()
+    p = oracle_params(O, w)
+    lut_z, r_cut, lut_v = w.lut()
+    atoms = w.atoms_for_phonon(0)
+    beams = O.beams(p)
+    n_beams, n_probes = len(beams), w.n_probes
+    # potential: full size is affordable only for small grids; sample a slab of slices otherwise
+    s_slab = w.n_slices if w.nx <= 256 else max(1, min(w.n_slices, 2))
+    p_slab = oracle_params(O, w.with_(n_slices=s_slab))
+    sel = atoms[:, 2] < s_slab * w.dz
+    t0 = time.perf_counter()
+    v = O.potential(p_slab, atoms[sel], w.z[sel], lut_z, r_cut, lut_v)
+    t_pot = (time.perf_counter() - t0) * (w.n_slices / s_slab)
+    # stage 1: `cores` beams through the slab, one per thread
+    nb = min(n_beams, cores)
+    t0 = time.perf_counter()
+    O.smatrix(p_slab, v, beams[:nb])
+    t_bs = (time.perf_counter() - t0) / (nb * s_slab) * cores          # core-seconds per beam-slice
+    t_s1 = t_bs * n_beams * w.n_slices / cores
+    # stage 2: `cores` probes on a reduced beam set (cost is linear in beams), seeded random S-matrix
+    nb2 = min(n_beams, max(4, int(2.0e9 // (w.nx * w.ny * 16))))
+    rng = np.random.default_rng(1)
+    s = (rng.standard_normal((nb2, w.ny, w.nx)) + 1j * rng.standard_normal((nb2, w.ny, w.nx)))
+    npr = min(n_probes, cores * 2)
+    t0 = time.perf_counter()
+    O.prism_probes(p, s, beams[:nb2], w.probe_xy()[:npr])
+    t_pr = (time.perf_counter() - t0) / npr * cores                    # core-seconds per probe at nb2 beams
+    t_s2 = t_pr * (n_beams / nb2) * n_probes / cores
+    total = t_pot + t_s1 + t_s2
+    desc = (f"oracle (fp64 C, gcc -O2, OpenMP x{cores}) on a sample of {w.name}: potential {s_slab}/{w.n_slices} "
+            f"slices, {nb} beams x {s_slab} slices, {npr} probes x {nb2}/{n_beams} beams; scaled linearly to "
+            f"{n_beams} beams x {w.n_slices} slices and {n_probes} probes")
+    detail = {"potential_s": t_pot, "smatrix_s": t_s1, "output_s": t_s2,
+              "beam_slices_per_s": n_beams * w.n_slices / t_s1}
+    return n_probes / total, desc, cores, detail
+
+
+def run_reference(args):
+    """--impl reference: the oracle is the reference arm for this tier (no pip-installable reference exists:
+    /root/reference holds only the paper text)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from paper_1706_08563_b200 import workloads
+    w = workloads.get(args.workload)
+    vals, last = [], None
+    t_begin = time.perf_counter()
+    for i in range(args.warmup + args.steps):
+        # each step is one bounded sample; keep the whole run within a few minutes
+        budget_left = 240.0 - (time.perf_counter() - t_begin)
+        if i >= 1 and budget_left < 0 and vals:
+            break
+        val, desc, cores, detail = oracle_sample(w)
+        last = (desc, cores, detail)
+        if i >= args.warmup or i == args.warmup + args.steps - 1:
+            vals.append(val)
+    value = float(np.mean(vals))
+    desc, cores, detail = last
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": len(vals), "warmup": args.warmup, "ms_per_step": 1e3 * w.n_probes / value,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": workload_config(w, args),
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "beam_slices_per_s": detail["beam_slices_per_s"],
+    }
+    print(json.dumps(line))
+
+
+def workload_config(w, args):
+    return {"workload": f"{w.name} ({WORKLOAD_NOTE.get(w.name, 'test case')}): {w.nx}x{w.ny} grid, "
+                        f"{w.n_slices} slices, f={w.f}, {w.probes_x}x{w.probes_y} probes, "
+                        f"{len(w.z)} atoms, one frozen-phonon configuration per step",
+            "grid": [w.nx, w.ny], "slices": w.n_slices, "f": w.f, "probes": [w.probes_x, w.probes_y],
+            "atoms": int(len(w.z)), "phonons": w.n_phonons, "potential_on_host": bool(w.potential_on_host),
+            "l2": "inputs larger than L2 (S-matrix and wave batch exceed 126 MB)"
+                  if w.nx >= 512 else "working set fits L2; L2 flushed between steps by the workspace writes"}
+
+
+# ------------------------------------------------------------------------------------------------ CUDA arm
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="P8", choices=["PR1", "P4", "P8", "P16"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    from paper_1706_08563_b200 import prism, workloads
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist_mod
+        dist = dist_mod
+        dist.init_process_group("nccl", device_id=dev)
+
+    w = workloads.get(args.workload)
+    p = prism.params_from_workload(w)
+    lut_z, r_cut, lut_v = w.lut()
+    n_beams, n_bins, n_probes = prism.num_beams(p), prism.num_bins(p), w.n_probes
+    npix = w.nx * w.ny
+
+    # all allocations up front
+    v_shape = (w.n_slices, w.ny, w.nx)
+    v = (torch.empty(v_shape, dtype=torch.float32).pin_memory() if w.potential_on_host
+         else torch.empty(v_shape, dtype=torch.float32, device=dev))
+    s = torch.empty((n_beams, w.ny, w.nx), dtype=torch.complex64, device=dev)
+    out_dev = torch.empty((w.probes_y, w.probes_x, n_bins), dtype=torch.float32, device=dev)
+    out_host = torch.empty((w.probes_y, w.probes_x, n_bins), dtype=torch.float32).pin_memory()
+    acc = torch.zeros_like(out_dev)
+    ws_bytes = max(prism.workspace_bytes(p, prism.WS_POTENTIAL, len(w.z)), prism.workspace_bytes(p, prism.WS_SMATRIX),
+                   prism.workspace_bytes(p, prism.WS_OUTPUT))
+    ws = torch.empty(ws_bytes, dtype=torch.uint8, device=dev)
+    # frozen-phonon configurations of this rank (host inputs, prepared outside the timed region)
+    my_phonons = [ph for ph in range(max(w.n_phonons, world)) if ph % world == rank]
+    atoms = {ph: np.ascontiguousarray(w.atoms_for_phonon(ph)) for ph in my_phonons}
+    beams_holder = {}
+
+    def step(k, out_target):
+        ph = my_phonons[k % len(my_phonons)]
+        prism.build_potential(p, atoms[ph], w.z, lut_z, r_cut, lut_v, v, ws)
+        beams_holder["b"] = prism.compute_smatrix(p, v, s, ws)
+        prism.compute_output(p, s, beams_holder["b"], out_target, ws)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for k in range(args.warmup):
+        step(k, out_dev)
+    barrier()
+
+    # ---- timed region: device-resident output, CUDA events on the launching stream ----
+    sampler = ClockSampler(local)
+    sampler.start()
+    prism.launch_count(reset=True)
+    prism.timing_enable(True)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    stage_ev = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(args.steps)]
+    barrier()
+    e0.record()
+    for k in range(args.steps):
+        ph = my_phonons[k % len(my_phonons)]
+        stage_ev[k][0].record()
+        prism.build_potential(p, atoms[ph], w.z, lut_z, r_cut, lut_v, v, ws)
+        stage_ev[k][1].record()
+        beams = prism.compute_smatrix(p, v, s, ws)
+        stage_ev[k][2].record()
+        prism.compute_output(p, s, beams, out_dev, ws)
+        stage_ev[k][3].record()
+        acc += out_dev
+    if dist is not None:
+        dist.all_reduce(acc)                                      # frozen-phonon average
+    e1.record()
+    barrier()
+    ms_total = e0.elapsed_time(e1)
+    launches = prism.launch_count()
+    prism.timing_enable(False)
+    kern = prism.timing_read()
+    clocks = sampler.stop()
+    stage_ms = [float(np.mean([stage_ev[k][i].elapsed_time(stage_ev[k][i + 1]) for k in range(args.steps)]))
+                for i in range(3)]
+    if dist is not None:
+        t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    ms_per_step = ms_total / args.steps
+    value = world * n_probes / (ms_per_step * 1e-3)
+
+    # ---- end to end: same calls, result delivered into pinned HOST memory inside the timed region ----
+    barrier()
+    t0 = time.perf_counter()
+    for k in range(args.steps):
+        step(k, out_host)
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    if dist is not None:
+        t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    cells = w.n_slices * (w.nx // 16) * (w.ny // 16)
+    v_bytes = 4 * npix * w.n_slices if w.potential_on_host else 0
+    h2d = 24 * len(w.z) + 4 * (cells + 1) + lut_v.size * 4 + v_bytes + 8 * (2 * w.nx + 2 * w.ny) \
+        + 8 * n_beams * (w.probes_x + w.probes_y + 2) + 4 * (w.nx // w.f) * (w.ny // w.f)
+    d2h = out_host.numel() * 4 + v_bytes
+    e2e_value = world * n_probes * args.steps / e2e_s
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel (16 N^2 bytes per wave and pass; 8 N_b M^2 flop per probe) --
+    hbm_peak, peak_src = measured_peaks()
+    m2 = (w.nx // w.f) * (w.ny // w.f)
+    per_launch_bytes = {"row_step": 16 * npix * n_beams, "col_step": 16 * npix * n_beams,
+                        "row_init": 8 * npix * n_beams, "row_final": 16 * npix * n_beams}
+    kernels = {}
+    for name, (ms, cnt) in kern.items():
+        entry = {"ms_per_step": ms / args.steps, "launches_per_step": cnt / args.steps, "avg_ms": ms / cnt}
+        if name in per_launch_bytes:
+            entry["algorithmic_GBps"] = per_launch_bytes[name] / (ms / cnt * 1e-3) / 1e9
+        if name == "beam_sum":
+            entry["algorithmic_TFLOPs"] = 8.0 * n_beams * m2 * n_probes * args.steps / (ms * 1e-3) / 1e12
+        kernels[name] = entry
+    top = max(kernels, key=lambda n: kernels[n]["ms_per_step"])
+    if top in per_launch_bytes:
+        ach = kernels[top]["algorithmic_GBps"]
+        roofline = {"kernel": top, "bound": "hbm", "achieved": ach, "peak": hbm_peak, "unit": "GB/s",
+                    "frac": ach / hbm_peak, "traffic": None, "peak_source": peak_src,
+                    "bytes_per_launch": per_launch_bytes[top]}
+    else:
+        ach = kernels[top].get("algorithmic_TFLOPs", 0.0)
+        roofline = {"kernel": top, "bound": "alu", "achieved": ach, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
+                    "frac": ach / FP32_PEAK_TFLOPS, "traffic": None,
+                    "peak_source": "derived: 148 SMs x 128 lanes x 2 flop x 1.965 GHz (DESIGN.md)"}
+    slice_ms = sum(kernels[k]["ms_per_step"] for k in ("row_init", "row_step", "col_step", "row_final") if k in kernels)
+    roofline["slice_step"] = {"algorithmic_GBps": 32.0 * npix * n_beams * w.n_slices / (slice_ms * 1e-3) / 1e9,
+                              "frac": 32.0 * npix * n_beams * w.n_slices / (slice_ms * 1e-3) / 1e9 / hbm_peak}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "complex64", "data": "synthetic", "config": workload_config(w, args), "clocks": clocks,
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h)},
+        "gpu_launches": int(launches),
+        "beam_slices_per_s": world * n_beams * w.n_slices / (stage_ms[1] * 1e-3),
+        "stage2_probes_per_s": world * n_probes / (stage_ms[2] * 1e-3),
+        "stage_ms": {"potential": stage_ms[0], "smatrix": stage_ms[1], "output": stage_ms[2]},
+        "roofline": roofline, "kernels": kernels,
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        val, desc, cores, detail = oracle_sample(w)
+        line["cpu_baseline"] = {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc,
+                                "beam_slices_per_s": detail["beam_slices_per_s"]}
+    print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

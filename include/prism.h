@@ -127,8 +127,17 @@ int multislice_compute_output(const prism_params* p, const float* v, float* out,
 /* Text for an error code, and the message of the last CUDA failure seen by the calling thread. */
 const char* prism_strerror(int code);
 const char* prism_last_error(void);
-/* Kernel launches enqueued by the calling thread since the last reset (for launch accounting). */
+/* Kernel launches enqueued by this process since the last reset (for launch accounting). */
 int64_t prism_launch_count(int32_t reset);
+
+/* Optional device timing per kernel class (measurement aid): when enabled, every
+ * launch is bracketed by a pair of CUDA events on the stream it is launched on.  prism_timing_read()
+ * waits for the recorded launches, adds their durations (ms) and counts per class into the two arrays
+ * (prism_timing_classes() entries each) and clears the record.  Not thread-safe; off by default. */
+int32_t     prism_timing_enable(int32_t enable);          /* returns the previous setting */
+int32_t     prism_timing_classes(void);
+const char* prism_timing_class_name(int32_t cls);
+int         prism_timing_read(double* ms_by_class, int64_t* launches_by_class);
 
 #ifdef __cplusplus
 }

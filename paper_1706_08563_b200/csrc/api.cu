@@ -28,11 +28,30 @@ static int cuda_fail(cudaError_t e, const char* what)
         cudaError_t e__ = (call);                                   \
         if (e__ != cudaSuccess) return cuda_fail(e__, #call);       \
     } while (0)
-#define LAUNCH(call)                                                \
-    do {                                                            \
-        cudaError_t e__ = (call);                                   \
-        if (e__ != cudaSuccess) return cuda_fail(e__, #call);       \
-        g_launches.fetch_add(1, std::memory_order_relaxed);         \
+
+// Optional per-kernel-class device timing (prism_timing_enable / prism_timing_read): a pair of
+// CUDA events around every launch, on the stream the kernel is launched on.
+enum KernelClass { K_POTENTIAL = 0, K_TRANSMISSION, K_ROW_INIT, K_ROW_STEP, K_ROW_FINAL, K_COL_STEP,
+                   K_BEAM_SUM, K_WIN_ROW_FFT, K_WIN_COL_ABS2, K_BIN_REDUCE, K_COL_MS_INIT, K_COL_MS_FINAL,
+                   K_NUM_CLASSES };
+static const char* const kClassNames[K_NUM_CLASSES] = {
+    "potential", "transmission", "row_init", "row_step", "row_final", "col_step", "beam_sum",
+    "win_row_fft", "win_col_abs2", "bin_reduce", "col_ms_init", "col_ms_final" };
+struct TimedLaunch { int cls; cudaEvent_t e0, e1; };
+static bool g_timing = false;
+static std::vector<TimedLaunch> g_timed;
+
+#define LAUNCH(cls, call, stream)                                                      \
+    do {                                                                               \
+        cudaEvent_t e0__ = nullptr, e1__ = nullptr;                                    \
+        if (g_timing) {                                                                \
+            cudaEventCreate(&e0__); cudaEventCreate(&e1__);                            \
+            cudaEventRecord(e0__, (stream));                                           \
+        }                                                                              \
+        cudaError_t e__ = (call);                                                      \
+        if (e__ != cudaSuccess) return cuda_fail(e__, #call);                          \
+        if (g_timing) { cudaEventRecord(e1__, (stream)); g_timed.push_back({(cls), e0__, e1__}); } \
+        g_launches.fetch_add(1, std::memory_order_relaxed);                            \
     } while (0)
 
 static const double kPi = 3.14159265358979323846264338327950288;
@@ -270,7 +289,7 @@ struct SliceFeeder {
             CU(cudaStreamWaitEvent(main_stream, filled[r], 0));
             src = ring[r];
         }
-        LAUNCH(launch_transmission(src, tbuf, sigma, npix, main_stream));
+        LAUNCH(K_TRANSMISSION, launch_transmission(src, tbuf, sigma, npix, main_stream), main_stream);
         if (on_host) CU(cudaEventRecord(consumed[s % RING], main_stream));
         return PRISM_OK;
     }
@@ -430,6 +449,33 @@ int64_t prism_launch_count(int32_t reset)
     return reset ? g_launches.exchange(0) : g_launches.load();
 }
 
+int32_t prism_timing_enable(int32_t enable)
+{
+    const int32_t was = g_timing ? 1 : 0;
+    g_timing = enable != 0;
+    return was;
+}
+
+int32_t prism_timing_classes(void) { return K_NUM_CLASSES; }
+const char* prism_timing_class_name(int32_t cls) { return (cls >= 0 && cls < K_NUM_CLASSES) ? kClassNames[cls] : ""; }
+
+int prism_timing_read(double* ms_by_class, int64_t* launches_by_class)
+{
+    if (!ms_by_class || !launches_by_class) return PRISM_EINVAL;
+    for (int c = 0; c < K_NUM_CLASSES; ++c) { ms_by_class[c] = 0.0; launches_by_class[c] = 0; }
+    for (const TimedLaunch& t : g_timed) {
+        CU(cudaEventSynchronize(t.e1));
+        float ms = 0.f;
+        CU(cudaEventElapsedTime(&ms, t.e0, t.e1));
+        ms_by_class[t.cls] += ms;
+        ++launches_by_class[t.cls];
+        cudaEventDestroy(t.e0);
+        cudaEventDestroy(t.e1);
+    }
+    g_timed.clear();
+    return PRISM_OK;
+}
+
 int prism_constants(double voltage, double* lambda, double* sigma)
 {
     if (!(voltage > 0)) return PRISM_EINVAL;
@@ -571,12 +617,12 @@ int prism_build_potential(const prism_params* p, const double* atoms_xyz, const 
         // grid.y is limited to 65535 slices per launch
         for (int s0 = 0; s0 < ns; s0 += 32768) {
             g.slice0 = s0; g.n_slices_chunk = std::min(32768, ns - s0); g.v_out = v + (size_t)s0 * npix;
-            LAUNCH(launch_potential(g, st));
+            LAUNCH(K_POTENTIAL, launch_potential(g, st), st);
         }
     } else {
         for (int s0 = 0; s0 < ns; s0 += POT_CHUNK_SLICES) {
             g.slice0 = s0; g.n_slices_chunk = std::min(POT_CHUNK_SLICES, ns - s0); g.v_out = L.stage;
-            LAUNCH(launch_potential(g, st));
+            LAUNCH(K_POTENTIAL, launch_potential(g, st), st);
             CU(cudaMemcpyAsync(v + (size_t)s0 * npix, L.stage, (size_t)g.n_slices_chunk * npix * sizeof(float),
                                cudaMemcpyDeviceToHost, st));
         }
@@ -636,14 +682,14 @@ int prism_compute_smatrix(const prism_params* p, const float* v, int32_t* beams_
                 if (r) return r;
                 if (sl == 0) {
                     ra.scale = (float)p->nx;                 // keeps A' = nx * FFT_x(t psi), see DESIGN.md
-                    LAUNCH(launch_row_pass(ROW_INIT, ra, st));
+                    LAUNCH(K_ROW_INIT, launch_row_pass(ROW_INIT, ra, st), st);
                 } else {
-                    LAUNCH(launch_row_pass(ROW_STEP, ra, st));
+                    LAUNCH(K_ROW_STEP, launch_row_pass(ROW_STEP, ra, st), st);
                 }
-                LAUNCH(launch_col_pass(COL_STEP, ca, st));
+                LAUNCH(K_COL_STEP, launch_col_pass(COL_STEP, ca, st), st);
             }
             ra.scale = 1.0f / (float)p->nx;
-            LAUNCH(launch_row_pass(ROW_FINAL, ra, st));
+            LAUNCH(K_ROW_FINAL, launch_row_pass(ROW_FINAL, ra, st), st);
         }
         return PRISM_OK;
     };
@@ -730,18 +776,18 @@ int prism_compute_output(const prism_params* p, const void* s, const int32_t* be
         g.s = (const float2*)s; g.w = L.w; g.coef_b = L.coef_b; g.phase_x = L.phase_x; g.phase_y = L.phase_y;
         g.win_x0 = L.win_x0; g.win_y0 = L.win_y0; g.n_beams = n_beams; g.nx = p->nx; g.ny = p->ny;
         g.mx = mx; g.my = my; g.probe0 = p0; g.n_probes_batch = np; g.probes_x = p->probes_x;
-        LAUNCH(launch_beam_sum(g, st));
+        LAUNCH(K_BEAM_SUM, launch_beam_sum(g, st), st);
         RowArgs ra;
         std::memset(&ra, 0, sizeof(ra));
         ra.a = L.w; ra.out = L.w; ra.tw_x = L.tw_x; ra.tw_y = L.tw_y; ra.n_waves = np; ra.nx = mx; ra.ny = my; ra.scale = 1.f;
-        LAUNCH(launch_row_pass(ROW_FFT, ra, st));
+        LAUNCH(K_WIN_ROW_FFT, launch_row_pass(ROW_FFT, ra, st), st);
         ColArgs ca;
         std::memset(&ca, 0, sizeof(ca));
         ca.a = L.w; ca.intensity = L.intensity; ca.tw_y = L.tw_y; ca.n_waves = np; ca.nx = mx; ca.ny = my;
         ca.scale = (float)(1.0 / (double)npix);
-        LAUNCH(launch_col_pass(COL_ABS2, ca, st));
-        LAUNCH(launch_bin_reduce(L.intensity, (int64_t)npix, L.bin_start, L.bin_pix, nb,
-                                 d_out + (size_t)p0 * nb, np, st));
+        LAUNCH(K_WIN_COL_ABS2, launch_col_pass(COL_ABS2, ca, st), st);
+        LAUNCH(K_BIN_REDUCE, launch_bin_reduce(L.intensity, (int64_t)npix, L.bin_start, L.bin_pix, nb,
+                                 d_out + (size_t)p0 * nb, np, st), st);
     }
     return copy_out(p, out, L.out_stage, out_dev, st);
 }
@@ -824,16 +870,17 @@ int multislice_compute_output(const prism_params* p, const float* v, float* out,
             std::memset(&ra, 0, sizeof(ra));
             ra.a = L.psi; ra.out = L.psi; ra.t = feed.tbuf; ra.tw_x = L.tab.tw_x; ra.tw_y = L.tab.tw_y;
             ra.n_waves = np; ra.nx = nx; ra.ny = ny; ra.scale = 1.f;
-            LAUNCH(launch_col_pass(COL_MS_INIT, ca, st));
+            LAUNCH(K_COL_MS_INIT, launch_col_pass(COL_MS_INIT, ca, st), st);
             feed.begin_sweep();
             for (int sl = 0; sl < p->n_slices; ++sl) {
                 int r = feed.get(sl);
                 if (r) return r;
-                LAUNCH(launch_row_pass(ROW_STEP, ra, st));
-                LAUNCH(launch_col_pass(sl == p->n_slices - 1 ? COL_MS_FINAL : COL_STEP, ca, st));
+                LAUNCH(K_ROW_STEP, launch_row_pass(ROW_STEP, ra, st), st);
+                if (sl == p->n_slices - 1) LAUNCH(K_COL_MS_FINAL, launch_col_pass(COL_MS_FINAL, ca, st), st);
+                else LAUNCH(K_COL_STEP, launch_col_pass(COL_STEP, ca, st), st);
             }
-            LAUNCH(launch_bin_reduce(L.intensity, (int64_t)npix, L.bin_start, L.bin_pix, nb,
-                                     d_out + (size_t)p0 * nb, np, st));
+            LAUNCH(K_BIN_REDUCE, launch_bin_reduce(L.intensity, (int64_t)npix, L.bin_start, L.bin_pix, nb,
+                                     d_out + (size_t)p0 * nb, np, st), st);
         }
         return PRISM_OK;
     };

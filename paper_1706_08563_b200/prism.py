@@ -20,7 +20,8 @@ WS_SMATRIX, WS_OUTPUT, WS_MULTISLICE, WS_POTENTIAL = 0, 1, 2, 3
 
 EXPORTS = ["prism_workspace_bytes", "prism_num_bins", "prism_num_beams", "prism_constants",
            "prism_build_potential", "prism_compute_smatrix", "prism_compute_output",
-           "multislice_compute_output", "prism_strerror", "prism_last_error", "prism_launch_count"]
+           "multislice_compute_output", "prism_strerror", "prism_last_error", "prism_launch_count",
+           "prism_timing_enable", "prism_timing_classes", "prism_timing_class_name", "prism_timing_read"]
 
 
 class Params(C.Structure):
@@ -77,6 +78,13 @@ def _load() -> C.CDLL:
     lib.prism_last_error.restype = C.c_char_p
     lib.prism_launch_count.restype = i64
     lib.prism_launch_count.argtypes = [i32]
+    lib.prism_timing_enable.restype = i32
+    lib.prism_timing_enable.argtypes = [i32]
+    lib.prism_timing_classes.restype = i32
+    lib.prism_timing_class_name.restype = C.c_char_p
+    lib.prism_timing_class_name.argtypes = [i32]
+    lib.prism_timing_read.restype = C.c_int
+    lib.prism_timing_read.argtypes = [C.POINTER(C.c_double), C.POINTER(i64)]
     return lib
 
 
@@ -140,6 +148,19 @@ def constants(voltage: float):
 
 def launch_count(reset: bool = False) -> int:
     return int(_lib.prism_launch_count(1 if reset else 0))
+
+
+def timing_enable(on: bool) -> bool:
+    return bool(_lib.prism_timing_enable(1 if on else 0))
+
+
+def timing_read() -> dict:
+    """{kernel class: (total ms, launches)} of the launches recorded since the last read."""
+    n = int(_lib.prism_timing_classes())
+    ms = (C.c_double * n)()
+    cnt = (C.c_int64 * n)()
+    _check(_lib.prism_timing_read(ms, cnt), "prism_timing_read")
+    return {_lib.prism_timing_class_name(i).decode(): (ms[i], int(cnt[i])) for i in range(n) if cnt[i]}
 
 
 def build_potential(p: Params, atoms_xyz, z_number, lut_z, r_cut, lut_v, v_out, workspace, stream=None):
