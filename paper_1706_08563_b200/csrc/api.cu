@@ -33,10 +33,10 @@ static int cuda_fail(cudaError_t e, const char* what)
 // CUDA events around every launch, on the stream the kernel is launched on.
 enum KernelClass { K_POTENTIAL = 0, K_TRANSMISSION, K_ROW_INIT, K_ROW_STEP, K_ROW_FINAL, K_COL_STEP,
                    K_BEAM_SUM, K_WIN_ROW_FFT, K_WIN_COL_ABS2, K_BIN_REDUCE, K_COL_MS_INIT, K_COL_MS_FINAL,
-                   K_NUM_CLASSES };
+                   K_LATTICE_DFT, K_NUM_CLASSES };
 static const char* const kClassNames[K_NUM_CLASSES] = {
     "potential", "transmission", "row_init", "row_step", "row_final", "col_step", "beam_sum",
-    "win_row_fft", "win_col_abs2", "bin_reduce", "col_ms_init", "col_ms_final" };
+    "win_row_fft", "win_col_abs2", "bin_reduce", "col_ms_init", "col_ms_final", "lattice_dft" };
 struct TimedLaunch { int cls; cudaEvent_t e0, e1; };
 static bool g_timing = false;
 static std::vector<TimedLaunch> g_timed;
@@ -353,9 +353,10 @@ static void layout_smatrix(Arena& a, const prism_params* p, int n_beams, Smatrix
     L.beams = a.take<int2>(n_beams);
 }
 
+constexpr int LATTICE_MAX_SLOTS = 4, LATTICE_MAX_Q = 32;
 struct OutputLayout {
-    float2 *tw_x, *tw_y, *coef_b, *phase_x, *phase_y, *w;
-    int *win_x0, *win_y0, *bin_start, *bin_pix;
+    float2 *tw_x, *tw_y, *coef_b, *phase_x, *phase_y, *w, *lat_coef;
+    int *win_x0, *win_y0, *bin_start, *bin_pix, *cell_beam;
     float *intensity, *out_stage;
     int batch;
 };
@@ -373,9 +374,57 @@ static void layout_output(Arena& a, const prism_params* p, int n_beams, OutputLa
     L.win_y0 = a.take<int>(p->probes_y);
     L.bin_start = a.take<int>(nb + 1);
     L.bin_pix = a.take<int>(npix);
+    L.lat_coef = a.take<float2>(n_beams);
+    L.cell_beam = a.take<int>((size_t)LATTICE_MAX_SLOTS * LATTICE_MAX_Q * LATTICE_MAX_Q);
     L.w = a.take<float2>((size_t)L.batch * npix);
     L.intensity = a.take<float>((size_t)L.batch * npix);
     L.out_stage = a.take<float>((size_t)p->probes_x * p->probes_y * nb);
+}
+
+// Regular probe lattice test ("lattice DFT"): the window origins advance by a constant
+// power-of-two number of pixels s that divides the window, the probe step is exactly s pixels, and every
+// beam index is a multiple of f.  Decided on the integer origin tables and in fp64.
+struct LatticePlan {
+    bool ok = false;
+    int q = 0, sx_log2 = 0, sy_log2 = 0, n_slots = 0;
+    std::vector<int> cell_beam;
+};
+static int regular_step(const std::vector<int>& w0, int n, int m, double step_px)
+{
+    if (w0.size() < 2) return 0;
+    const int s = ((w0[1] - w0[0]) % n + n) % n;
+    if (s < 1 || !is_pow2(s) || m % s) return 0;
+    for (size_t i = 1; i < w0.size(); ++i)
+        if ((((w0[i] - w0[i - 1]) % n) + n) % n != s) return 0;
+    if (std::fabs(step_px - (double)s) > 1e-9) return 0;
+    if ((long long)w0.size() * s > n) return 0;                   // every probe owns a distinct lattice site
+    return s;
+}
+static LatticePlan plan_lattice(const prism_params* p, const int32_t* beams, int n_beams,
+                                const std::vector<int>& wx0, const std::vector<int>& wy0, int mx, int my)
+{
+    LatticePlan L;
+    const int sx = regular_step(wx0, p->nx, mx, p->probe_step[0] / (p->cell[0] / p->nx));
+    const int sy = regular_step(wy0, p->ny, my, p->probe_step[1] / (p->cell[1] / p->ny));
+    if (!sx || !sy || mx / sx != my / sy) return L;
+    const int q = mx / sx;
+    if (q != 8 && q != 16 && q != 32) return L;
+    std::vector<int> count((size_t)q * q, 0);
+    L.cell_beam.assign((size_t)LATTICE_MAX_SLOTS * q * q, -1);
+    for (int b = 0; b < n_beams; ++b) {
+        const int kx = beams[2 * b], ky = beams[2 * b + 1];
+        if (kx % p->f || ky % p->f) return L;
+        const int m = ((kx / p->f) % q + q) % q, n = ((ky / p->f) % q + q) % q;
+        const int c = n * q + m;
+        if (count[c] >= LATTICE_MAX_SLOTS) return L;
+        L.cell_beam[(size_t)count[c] * q * q + c] = b;
+        L.n_slots = std::max(L.n_slots, ++count[c]);
+    }
+    for (L.sx_log2 = 0; (1 << L.sx_log2) < sx; ++L.sx_log2) {}
+    for (L.sy_log2 = 0; (1 << L.sy_log2) < sy; ++L.sy_log2) {}
+    L.q = q;
+    L.ok = L.n_slots >= 1;
+    return L;
 }
 
 struct MultisliceLayout {
@@ -767,16 +816,47 @@ int prism_compute_output(const prism_params* p, const void* s, const int32_t* be
     ring_lists(p, mx, my, p->f, p->f, bstart, bpix);
     CU(upload(L.bin_start, bstart, st));
     CU(upload(L.bin_pix, bpix, st));
+    // regular probe lattice: the beam sum of all probes is a Q x Q DFT per S-matrix pixel
+    LatticePlan lat = plan_lattice(p, beams, n_beams, wx0, wy0, mx, my);
+    const int rows_per_batch = L.batch / p->probes_x;
+    if (rows_per_batch < 1) lat.ok = false;
+    std::vector<float2> lcoef;
+    if (lat.ok) {
+        lcoef.resize(n_beams);
+        for (int b = 0; b < n_beams; ++b) {
+            const double qx = kxs[b] / p->cell[0], qy = kys[b] / p->cell[1];
+            double turns = kxs[b] * (p->probe_origin[0] / p->cell[0]) + kys[b] * (p->probe_origin[1] / p->cell[1]);
+            turns -= std::floor(turns);
+            const double ang = -aberration(p, lambda, qx * qx + qy * qy) - 2.0 * kPi * turns;
+            lcoef[b] = make_float2((float)(wscale * std::cos(ang)), (float)(wscale * std::sin(ang)));
+        }
+        CU(upload(L.lat_coef, lcoef, st));
+        CU(upload(L.cell_beam, lat.cell_beam, st));
+    }
     CU(cudaStreamSynchronize(st));          // host vectors above are local
 
     const int n_probes = p->probes_x * p->probes_y;
-    for (int p0 = 0; p0 < n_probes; p0 += L.batch) {
-        const int np = std::min(L.batch, n_probes - p0);
-        BeamSumArgs g;
-        g.s = (const float2*)s; g.w = L.w; g.coef_b = L.coef_b; g.phase_x = L.phase_x; g.phase_y = L.phase_y;
-        g.win_x0 = L.win_x0; g.win_y0 = L.win_y0; g.n_beams = n_beams; g.nx = p->nx; g.ny = p->ny;
-        g.mx = mx; g.my = my; g.probe0 = p0; g.n_probes_batch = np; g.probes_x = p->probes_x;
-        LAUNCH(K_BEAM_SUM, launch_beam_sum(g, st), st);
+    const int batch = lat.ok ? rows_per_batch * p->probes_x : L.batch;
+    for (int p0 = 0; p0 < n_probes; p0 += batch) {
+        const int np = std::min(batch, n_probes - p0);
+        if (lat.ok) {
+            LatticeArgs g;
+            g.s = (const float2*)s; g.w = L.w; g.coef = L.lat_coef; g.cell_beam = L.cell_beam;
+            g.n_slots = lat.n_slots; g.q = lat.q; g.nx = p->nx; g.ny = p->ny; g.mx = mx; g.my = my;
+            g.sx_log2 = lat.sx_log2; g.sy_log2 = lat.sy_log2; g.x00 = wx0[0]; g.y00 = wy0[0];
+            g.probes_x = p->probes_x; g.probes_y = p->probes_y;
+            g.py0 = p0 / p->probes_x; g.n_rows = np / p->probes_x;
+            const int sy = 1 << lat.sy_log2;
+            g.row0 = (int)(((long long)g.py0 * sy) % p->ny);
+            g.n_pix_rows = std::min(p->ny, sy * (g.n_rows - 1) + my);
+            LAUNCH(K_LATTICE_DFT, launch_lattice_dft(g, st), st);
+        } else {
+            BeamSumArgs g;
+            g.s = (const float2*)s; g.w = L.w; g.coef_b = L.coef_b; g.phase_x = L.phase_x; g.phase_y = L.phase_y;
+            g.win_x0 = L.win_x0; g.win_y0 = L.win_y0; g.n_beams = n_beams; g.nx = p->nx; g.ny = p->ny;
+            g.mx = mx; g.my = my; g.probe0 = p0; g.n_probes_batch = np; g.probes_x = p->probes_x;
+            LAUNCH(K_BEAM_SUM, launch_beam_sum(g, st), st);
+        }
         RowArgs ra;
         std::memset(&ra, 0, sizeof(ra));
         ra.a = L.w; ra.out = L.w; ra.tw_x = L.tw_x; ra.tw_y = L.tw_y; ra.n_waves = np; ra.nx = mx; ra.ny = my; ra.scale = 1.f;

@@ -99,6 +99,46 @@ template <> struct Dft<16> {
     }
 };
 
+template <> struct Dft<32> {
+    __device__ __forceinline__ static void run(float2* a)
+    {
+        // n = 4 n1 + n2 (n1 < 8, n2 < 4); k = k1 + 8 k2.  Y[n2][k1] = DFT8 over n1, twiddle w32^(n2 k1), DFT4 over n2.
+        // w32^m = exp(-2 pi i m / 32) = (WC[m], -WS[m]) for m <= 21
+        constexpr float WC[22] = { 1.f, 0.98078528040323044913f, 0.92387953251128675613f, 0.83146961230254523708f,
+                                   0.70710678118654752440f, 0.55557023301960222474f, 0.38268343236508977173f,
+                                   0.19509032201612826785f, 0.f, -0.19509032201612826785f, -0.38268343236508977173f,
+                                   -0.55557023301960222474f, -0.70710678118654752440f, -0.83146961230254523708f,
+                                   -0.92387953251128675613f, -0.98078528040323044913f, -1.f, -0.98078528040323044913f,
+                                   -0.92387953251128675613f, -0.83146961230254523708f, -0.70710678118654752440f,
+                                   -0.55557023301960222474f };
+        constexpr float WS[22] = { 0.f, 0.19509032201612826785f, 0.38268343236508977173f, 0.55557023301960222474f,
+                                   0.70710678118654752440f, 0.83146961230254523708f, 0.92387953251128675613f,
+                                   0.98078528040323044913f, 1.f, 0.98078528040323044913f, 0.92387953251128675613f,
+                                   0.83146961230254523708f, 0.70710678118654752440f, 0.55557023301960222474f,
+                                   0.38268343236508977173f, 0.19509032201612826785f, 0.f, -0.19509032201612826785f,
+                                   -0.38268343236508977173f, -0.55557023301960222474f, -0.70710678118654752440f,
+                                   -0.83146961230254523708f };
+        float2 y[4][8];
+#pragma unroll
+        for (int n2 = 0; n2 < 4; ++n2) {
+#pragma unroll
+            for (int n1 = 0; n1 < 8; ++n1) y[n2][n1] = a[4 * n1 + n2];
+            Dft<8>::run(y[n2]);
+        }
+#pragma unroll
+        for (int n2 = 1; n2 < 4; ++n2)
+#pragma unroll
+            for (int k1 = 1; k1 < 8; ++k1)
+                y[n2][k1] = cmul(y[n2][k1], make_float2(WC[n2 * k1], -WS[n2 * k1]));
+#pragma unroll
+        for (int k1 = 0; k1 < 8; ++k1) {
+            float2 z[4] = { y[0][k1], y[1][k1], y[2][k1], y[3][k1] };
+            Dft<4>::run(z);
+            a[k1] = z[0]; a[k1 + 8] = z[1]; a[k1 + 16] = z[2]; a[k1 + 24] = z[3];
+        }
+    }
+};
+
 // ---- plan ---------------------------------------------------------------------
 template <int N_, int E_, int R1_, int R2_, int R3_>
 struct Plan {

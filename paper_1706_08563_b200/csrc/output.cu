@@ -86,6 +86,143 @@ cudaError_t launch_beam_sum(const BeamSumArgs& g, cudaStream_t stream)
     return cudaGetLastError();
 }
 
+// =============================================================================
+// Lattice DFT (regular probe grids).  PAPER.md:86/:128 define probe p's window as
+//   w_p[j][i] = sum_b c_b exp(-2 pi i q_b . r_p) S_b[y0_p + j][x0_p + i].
+// With r_p = r_0 + (px, py) * step and step = s pixels (s | window M), beam b =
+// (f m_b, f n_b) gives exp(-2 pi i (m_b px + n_b py) / Q), Q = M / s: for a fixed
+// S-matrix pixel the values needed by ALL probes are the Q x Q forward DFT of the
+// beam lattice array G[n][m] = sum_{b folded onto (n, m) mod Q} c'_b S_b[y][x], and
+// the pixel lies in the window of exactly one probe per residue class.  One CTA
+// takes TP = 8 * 32/Q pixels of a row: (1) gather + fold + scale into shared
+// memory with coalesced reads of S, (2) one warp per 32/Q pixels runs the row and
+// column FFT_Q in registers (lane = lattice row / column), (3) the results are
+// scattered to the windows, contiguous runs of pixels going to the same probe.
+// =============================================================================
+template <int Q> struct LatticeCfg {
+    static constexpr int PW = 32 / Q;                 // pixels per warp
+    static constexpr int TP = 8 * PW;                 // pixels per CTA (256 threads)
+    static constexpr int RS = Q + 1;                  // padded row stride (complex)
+    static constexpr int PS = Q * RS + (Q == 32 ? 2 : 1);   // pixel stride: conflict-free for phases 1 and 3
+    static constexpr size_t SMEM = (size_t)TP * PS * sizeof(float2);
+};
+
+template <int Q>
+__global__ void __launch_bounds__(256, 2) lattice_dft_kernel(LatticeArgs g)
+{
+    using C = LatticeCfg<Q>;
+    constexpr int TP = C::TP, RS = C::RS, PS = C::PS, CPI = 256 / TP;   // cells per iteration
+    extern __shared__ float2 sm[];                    // [TP][PS]
+    const int tid = threadIdx.x;
+    const int tiles_x = g.nx / TP;
+    const int r = blockIdx.x / tiles_x, xt = (blockIdx.x % tiles_x) * TP;
+    const int yp = (g.row0 + r) & (g.ny - 1);         // row relative to the first window origin
+    const int y = (yp + g.y00) & (g.ny - 1);
+    const int px = tid % TP, c0 = tid / TP;
+
+    // ---- (1) G[n][m] = sum over folded beams of c'_b S_b[y][x] ----
+    {
+        const size_t layer = (size_t)g.nx * g.ny;
+        const float2* src = g.s + (size_t)y * g.nx + xt + px;
+        float2* dst = sm + px * PS;
+        if (g.n_slots == 1) {
+#pragma unroll 8
+            for (int c = c0; c < Q * Q; c += CPI) {
+                const int b = __ldg(g.cell_beam + c);
+                const float2 a = b >= 0 ? __ldg(g.coef + b) : make_float2(0.f, 0.f);
+                const float2 v = __ldg(src + (size_t)max(b, 0) * layer);
+                dst[(c / Q) * RS + (c % Q)] = cmul(a, v);
+            }
+        } else {
+#pragma unroll 2
+            for (int c = c0; c < Q * Q; c += CPI) {
+                float2 acc = make_float2(0.f, 0.f);
+                for (int sl = 0; sl < g.n_slots; ++sl) {
+                    const int b = __ldg(g.cell_beam + sl * Q * Q + c);
+                    const float2 a = b >= 0 ? __ldg(g.coef + b) : make_float2(0.f, 0.f);
+                    const float2 v = __ldg(src + (size_t)max(b, 0) * layer);
+                    acc = cadd(acc, cmul(a, v));
+                }
+                dst[(c / Q) * RS + (c % Q)] = acc;
+            }
+        }
+    }
+    __syncthreads();
+
+    // ---- (2) Q x Q forward DFT of every pixel's lattice array, in registers ----
+    {
+        const int warp = tid >> 5, lane = tid & 31;
+        const int rr = lane % Q;
+        float2* base = sm + (warp * C::PW + lane / Q) * PS;
+        float2 v[Q];
+#pragma unroll
+        for (int m = 0; m < Q; ++m) v[m] = base[rr * RS + m];           // lattice row n = rr
+        Dft<Q>::run(v);                                                  // over m -> probe residue in x
+#pragma unroll
+        for (int m = 0; m < Q; ++m) base[rr * RS + m] = v[m];
+        __syncwarp();
+#pragma unroll
+        for (int n = 0; n < Q; ++n) v[n] = base[n * RS + rr];           // column: residue x = rr
+        Dft<Q>::run(v);                                                  // over n -> probe residue in y
+        __syncwarp();
+#pragma unroll
+        for (int n = 0; n < Q; ++n) base[n * RS + rr] = v[n];
+    }
+    __syncthreads();
+
+    // ---- (3) scatter: residue (ry, rx) of this pixel belongs to the one probe of that class covering it ----
+    {
+        const int sx = g.sx_log2, sy = g.sy_log2;
+        const int xp = (xt + px - g.x00) & (g.nx - 1);
+        const int xc = xp >> sx, xin = xp & ((1 << sx) - 1);
+        const int yc = yp >> sy, yin = yp & ((1 << sy) - 1);
+        const int wrap_x = g.nx >> sx, wrap_y = g.ny >> sy;
+        const size_t npix = (size_t)g.mx * g.my;
+        const float2* srcp = sm + px * PS;
+#pragma unroll 4
+        for (int c = c0; c < Q * Q; c += CPI) {
+            const int ry = c / Q, rx = c % Q;
+            const int u = (xc - rx) & (Q - 1), v = (yc - ry) & (Q - 1);
+            int pp = xc - u, pq = yc - v;
+            if (pp < 0) pp += wrap_x;
+            if (pq < 0) pq += wrap_y;
+            const int prow = pq - g.py0;
+            if (pp < g.probes_x && prow >= 0 && prow < g.n_rows) {
+                const int i = (u << sx) + xin, j = (v << sy) + yin;
+                g.w[((size_t)prow * g.probes_x + pp) * npix + (size_t)j * g.mx + i] = srcp[ry * RS + rx];
+            }
+        }
+    }
+}
+
+template <int Q>
+static cudaError_t launch_lattice_q(const LatticeArgs& g, cudaStream_t stream)
+{
+    using C = LatticeCfg<Q>;
+    static bool set = false;
+    if (!set) {
+        cudaError_t e = cudaFuncSetAttribute(lattice_dft_kernel<Q>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
+        if (e != cudaSuccess) return e;
+        set = true;
+    }
+    if (g.nx % C::TP) return cudaErrorInvalidValue;
+    const long long blocks = (long long)(g.nx / C::TP) * g.n_pix_rows;
+    if (blocks <= 0) return cudaSuccess;
+    if (blocks > 0x7fffffffLL) return cudaErrorInvalidValue;
+    lattice_dft_kernel<Q><<<(unsigned)blocks, 256, C::SMEM, stream>>>(g);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_lattice_dft(const LatticeArgs& g, cudaStream_t stream)
+{
+    switch (g.q) {
+        case 8:  return launch_lattice_q<8>(g, stream);
+        case 16: return launch_lattice_q<16>(g, stream);
+        case 32: return launch_lattice_q<32>(g, stream);
+    }
+    return cudaErrorInvalidValue;
+}
+
 // Annular-ring integration: one CTA per wave, one warp per ring at a time; the
 // pixels of each ring are listed by the host (fp64 bin decisions), and are summed
 // in a fixed order, so the result is deterministic.

@@ -68,6 +68,25 @@ struct BeamSumArgs {
 };
 cudaError_t launch_beam_sum(const BeamSumArgs& args, cudaStream_t stream);
 
+// Regular probe lattice (probe step = 2^k pixels dividing the window): for one S-matrix pixel the
+// probe phases exp(-2 pi i q_b . r_p) over the probe lattice are a Q x Q DFT over the beam lattice
+// (Q = window / step), so all Q^2 probes whose windows hold that pixel are served by one small
+// 2-D FFT instead of Q^2 separate beam sums (same sums, reordered).
+struct LatticeArgs {
+    const float2* s;          // [n_beams][ny][nx] compact S-matrix
+    float2*       w;          // [n_rows * probes_x][my][mx] summed windows of the batch (out)
+    const float2* coef;       // [n_beams] A_b exp(-i chi_b) * scale * exp(-2 pi i q_b . r_probe0)
+    const int*    cell_beam;  // [n_slots][q * q]: beams folded onto lattice residue (ky/f mod q, kx/f mod q); -1 = none
+    int           n_slots, q;
+    int           nx, ny, mx, my;
+    int           sx_log2, sy_log2;   // probe step in pixels = 1 << s_log2
+    int           x00, y00;           // window origin of probe (0, 0), wrapped
+    int           probes_x, probes_y;
+    int           py0, n_rows;        // probe rows [py0, py0 + n_rows) of this batch
+    int           row0, n_pix_rows;   // pixel rows y' = (row0 + r) mod ny, r < n_pix_rows, y' relative to y00
+};
+cudaError_t launch_lattice_dft(const LatticeArgs& args, cudaStream_t stream);
+
 // out[w][bin] = sum of intensity[w][pix] over the pixels listed for the bin (CSR), fixed order
 cudaError_t launch_bin_reduce(const float* intensity, int64_t npix, const int* bin_start,
                               const int* bin_pix, int n_bins, float* out, int n_waves,

@@ -100,6 +100,62 @@ def test_multislice_parity(G, name):
     assert rel_l2(out[:, d:], ref[:, d:]) < 5 * TOL_OUT
 
 
+# ---- regular probe lattices: the lattice-DFT form of the beam sum -----------------
+def _lattice_cases():
+    return {
+        # Q = 8, off-pixel origin, 64^2 windows
+        "L128f2q8": W.scaled_test_case(128, 3, 2, 16, alpha_mrad=25.0, defocus=30.0, seed_index=11,
+                                       probe_offset=(0.137, 0.291)),
+        # Q = 32 with 128^2 windows and a 4-pixel step: the shape of BASELINE.json configs 3-5
+        "L256f2q32": W.scaled_test_case(256, 3, 2, 64, voltage=300e3, alpha_mrad=20.0, seed_index=12),
+        # Q = 16
+        "L256f4q16": W.scaled_test_case(256, 2, 4, 64, voltage=300e3, alpha_mrad=20.0, seed_index=13, cs=1.0e4),
+        # Q = 16 with beams folded onto the same lattice residue (25 beam indices per axis onto 16)
+        "L128f1q16": W.scaled_test_case(128, 2, 1, 16, alpha_mrad=25.0, seed_index=14, density=0.03),
+        # probe grid covering part of the cell only, rectangular, origin away from 0
+        "L128f2part": W.scaled_test_case(128, 2, 2, 16, alpha_mrad=20.0, seed_index=15).with_(
+            probes_x=5, probes_y=7, probe_origin=(1.2, 3.3)),
+    }
+
+
+LATTICE = _lattice_cases()
+
+
+@pytest.mark.parametrize("name", list(LATTICE))
+def test_prism_output_parity_regular_lattice(G, name):
+    w = LATTICE[name]
+    p = oracle_params(w)
+    v = G.gpu_potential(w)
+    s, beams = G.gpu_smatrix(w, v)
+    out = G.gpu_prism_output(w, s, beams)
+    xy = w.probe_xy()
+    pick = np.unique(np.linspace(0, len(xy) - 1, 97).astype(int))       # oracle on a spread of probes
+    s_ref = O.smatrix(p, oracle_potential(w), beams)
+    ref = O.prism_probes(p, s_ref, beams, xy[pick])
+    assert rel_l2(out[pick], ref) < TOL_OUT
+    d = G.dark_field(w, p)
+    assert ref[:, d:].sum() > 0
+    assert rel_l2(out[pick][:, d:], ref[:, d:]) < 5 * TOL_OUT
+    # the stage in isolation: oracle stage 2 applied to the GPU's own S-matrix, every probe row touched
+    rows = np.unique(np.concatenate([np.arange(0, len(xy), 53), [len(xy) - 1]]))
+    ref2 = O.prism_probes(p, s.cpu().numpy().astype(np.complex128), beams, xy[rows])
+    assert rel_l2(out[rows], ref2) < 2e-5
+
+
+def test_lattice_path_does_not_depend_on_batch(G):
+    from paper_1706_08563_b200 import prism
+    w = LATTICE["L128f2part"]
+    v = G.gpu_potential(w)
+    s, beams = G.gpu_smatrix(w, v)
+    out0 = G.gpu_prism_output(w, s, beams)
+    for b in [w.probes_x, 3 * w.probes_x + 2, 2]:           # one probe row, three rows, fewer than a row (direct sum)
+        out1 = G.gpu_prism_output(w, s, beams, prism.params_from_workload(w, batch=b))
+        if b >= w.probes_x:
+            assert np.array_equal(out0, out1)
+        else:
+            assert rel_l2(out1, out0) < 2e-5
+
+
 def test_prism_f1_equals_multislice_on_gpu(G):
     w = CASES["PR1"]
     v = G.gpu_potential(w)
