@@ -305,8 +305,11 @@ def main():
     # ---- roofline of the dominant kernel (16 N^2 bytes per wave and pass; 8 N_b M^2 flop per probe) --
     hbm_peak, peak_src = measured_peaks()
     m2 = (w.nx // w.f) * (w.ny // w.f)
-    per_launch_bytes = {"row_step": 16 * npix * n_beams, "col_step": 16 * npix * n_beams,
-                        "row_init": 8 * npix * n_beams, "row_final": 16 * npix * n_beams}
+    # algorithmic bytes per wave and pass: mixed space is moved for the 2c in-band columns of
+    # the nx only (c = prism_band_columns; whole waves below 256 points), real space in full
+    band = 2.0 * prism.band_columns(p) / w.nx if min(w.nx, w.ny) >= 256 else 1.0
+    mixed, real = 8 * npix * n_beams * band, 8 * npix * n_beams
+    per_launch_bytes = {"row_step": 2 * mixed, "col_step": 2 * mixed, "row_init": mixed, "row_final": mixed + real}
     kernels = {}
     for name, (ms, cnt) in kern.items():
         entry = {"ms_per_step": ms / args.steps, "launches_per_step": cnt / args.steps, "avg_ms": ms / cnt}
@@ -327,8 +330,14 @@ def main():
                     "frac": ach / FP32_PEAK_TFLOPS, "traffic": None,
                     "peak_source": "derived: 148 SMs x 128 lanes x 2 flop x 1.965 GHz (DESIGN.md)"}
     slice_ms = sum(kernels[k]["ms_per_step"] for k in ("row_init", "row_step", "col_step", "row_final") if k in kernels)
-    roofline["slice_step"] = {"algorithmic_GBps": 32.0 * npix * n_beams * w.n_slices / (slice_ms * 1e-3) / 1e9,
-                              "frac": 32.0 * npix * n_beams * w.n_slices / (slice_ms * 1e-3) / 1e9 / hbm_peak}
+    step_bytes = 4 * mixed * w.n_slices + real                       # S row+col passes of 2 * mixed each, one real-space store
+    flops = n_beams * w.n_slices * npix * (10.0 * (np.log2(w.nx) + np.log2(w.ny)) + 12.0)
+    roofline["slice_step"] = {"algorithmic_GBps": step_bytes / (slice_ms * 1e-3) / 1e9,
+                              "frac": step_bytes / (slice_ms * 1e-3) / 1e9 / hbm_peak,
+                              "band_fraction": band,
+                              "unbanded_32N2_GBps": 32.0 * npix * n_beams * w.n_slices / (slice_ms * 1e-3) / 1e9,
+                              "fp32_TFLOPs_nominal": flops / (slice_ms * 1e-3) / 1e12,
+                              "fp32_frac": flops / (slice_ms * 1e-3) / 1e12 / FP32_PEAK_TFLOPS}
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,

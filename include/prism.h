@@ -85,6 +85,11 @@ int32_t prism_num_bins(const prism_params* p);
  * scattering angle"): signed indices kx = 0 mod f, ky = 0 mod f with (kx/lx)^2 + (ky/ly)^2 <= (alpha/lambda)^2,
  * decided in fp64 on the host. */
 int     prism_num_beams(const prism_params* p, int32_t* n_beams);
+/* Columns of mixed space A[w][y][kx] that the slice step moves through HBM (host-only): the 2/3 band-limit of
+ * the propagator (BASELINE.json; reading R1) leaves kx in [0, c) and [nx - c, nx) only, c = the returned
+ * count (a multiple of 32, at most nx / 2), so one pass reads and writes 2 c / nx of a wave.  Grids below
+ * 256 points move whole waves (the return value still describes the band). */
+int32_t prism_band_columns(const prism_params* p);
 /* lambda (Angstrom) and sigma (rad / (V Angstrom)) used by the library for this voltage (host-only). */
 int     prism_constants(double voltage, double* lambda, double* sigma);
 

@@ -152,6 +152,17 @@ static void band_limit(const prism_params* p, std::vector<int>& ky_lim)
     }
 }
 
+// Columns of mixed space that can be non-zero: kx in [0, xband) and [nx - xband, nx), xband a multiple of 32
+// (tile widths of the pipelined column pass) that covers every kx with a non-empty band-limited column.
+static int band_columns(const prism_params* p)
+{
+    std::vector<int> lim;
+    band_limit(p, lim);
+    int kxmax = 0;
+    for (int m = 0; m <= p->nx / 2; ++m) if (lim[m] >= 0) kxmax = m;
+    return std::min(p->nx / 2, (kxmax + 1 + 31) / 32 * 32);
+}
+
 static double aberration(const prism_params* p, double lambda, double q2)
 {
     return kPi * lambda * q2 * p->defocus + 0.5 * kPi * p->cs * lambda * lambda * lambda * q2 * q2;
@@ -538,6 +549,12 @@ int32_t prism_num_bins(const prism_params* p)
     return (int32_t)std::floor(p->det_max / p->det_step + 0.5);
 }
 
+int32_t prism_band_columns(const prism_params* p)
+{
+    if (check_common(p)) return 0;
+    return band_columns(p);
+}
+
 int prism_num_beams(const prism_params* p, int32_t* n_beams)
 {
     if (!n_beams) return PRISM_EINVAL;
@@ -714,15 +731,17 @@ int prism_compute_smatrix(const prism_params* p, const float* v, int32_t* beams_
     if ((rc = feed.init())) { feed.release(); return rc; }
 
     const int batch = p->batch > 0 ? std::min<int>(p->batch, n_beams) : n_beams;
+    const int xband = band_columns(p);
     auto run = [&]() -> int {
         for (int b0 = 0; b0 < n_beams; b0 += batch) {
             const int nb = std::min(batch, n_beams - b0);
             RowArgs ra;
             ra.a = (float2*)s + (size_t)b0 * npix; ra.out = ra.a; ra.t = feed.tbuf;
             ra.tw_x = L.tab.tw_x; ra.tw_y = L.tab.tw_y; ra.beams = L.beams + b0;
-            ra.n_waves = nb; ra.nx = p->nx; ra.ny = p->ny; ra.scale = 1.f;
+            ra.n_waves = nb; ra.nx = p->nx; ra.ny = p->ny; ra.scale = 1.f; ra.xband = xband;
             ColArgs ca;
             std::memset(&ca, 0, sizeof(ca));
+            ca.xband = xband;
             ca.a = ra.a; ca.tw_y = L.tab.tw_y; ca.prop_x = L.tab.prop_x; ca.prop_y = L.tab.prop_y;
             ca.ky_lim = L.tab.ky_lim; ca.n_waves = nb; ca.nx = p->nx; ca.ny = p->ny; ca.scale = 1.f;
             feed.begin_sweep();
@@ -936,6 +955,10 @@ int multislice_compute_output(const prism_params* p, const float* v, float* out,
     if ((rc = feed.init())) { feed.release(); return rc; }
 
     const int n_probes = p->probes_x * p->probes_y;
+    const int xband = band_columns(p);
+    // the pipelined column pass writes the detector plane for in-band columns only: the rest stays zero (R12)
+    if (pipelined_grid(nx, ny))
+        CU(cudaMemsetAsync(L.intensity, 0, (size_t)L.batch * npix * sizeof(float), st));
     auto run = [&]() -> int {
         for (int p0 = 0; p0 < n_probes; p0 += L.batch) {
             const int np = std::min(L.batch, n_probes - p0);
@@ -944,12 +967,12 @@ int multislice_compute_output(const prism_params* p, const float* v, float* out,
             ca.a = L.psi; ca.intensity = L.intensity; ca.tw_y = L.tab.tw_y; ca.prop_x = L.tab.prop_x;
             ca.prop_y = L.tab.prop_y; ca.ky_lim = L.tab.ky_lim; ca.aperture_t = L.aperture_t;
             ca.phase_x = L.phase_x; ca.phase_y = L.phase_y; ca.probe0 = p0; ca.probes_x = p->probes_x;
-            ca.n_waves = np; ca.nx = nx; ca.ny = ny;
+            ca.n_waves = np; ca.nx = nx; ca.ny = ny; ca.xband = xband;
             ca.scale = (float)((double)ny / (double)nx);      // I = |Psi_S|^2 / (nx ny), see DESIGN.md
             RowArgs ra;
             std::memset(&ra, 0, sizeof(ra));
             ra.a = L.psi; ra.out = L.psi; ra.t = feed.tbuf; ra.tw_x = L.tab.tw_x; ra.tw_y = L.tab.tw_y;
-            ra.n_waves = np; ra.nx = nx; ra.ny = ny; ra.scale = 1.f;
+            ra.n_waves = np; ra.nx = nx; ra.ny = ny; ra.scale = 1.f; ra.xband = xband;
             LAUNCH(K_COL_MS_INIT, launch_col_pass(COL_MS_INIT, ca, st), st);
             feed.begin_sweep();
             for (int sl = 0; sl < p->n_slices; ++sl) {

@@ -164,7 +164,7 @@ template <> struct PlanFor<2048> { using type = Plan<2048, 16, 16, 16, 8>; };
 
 __device__ __forceinline__ int pad16(int i) { return i + (i >> 4); }
 
-// Per-thread twiddles, loaded once from the table tw[m] = exp(-2 pi i m / N).
+// Per-thread twiddles, loaded once from the table tw[m] = exp(-2 pi i m / N) and kept in registers.
 template <class P>
 struct Twiddles {
     float2 s2[P::S2_SETS][P::R2 > 1 ? P::R2 - 1 : 1];
@@ -189,33 +189,68 @@ struct Twiddles {
             }
         }
     }
+    __device__ __forceinline__ float2 get2(int m, int r) const { return s2[P::S2_SHARED ? 0 : m][r - 1]; }
+    __device__ __forceinline__ float2 get3(int m, int r) const { return s3[m][r - 1]; }
+};
+
+// The same twiddles kept in shared memory, transposed so that the threads of a line read consecutive
+// words:  t2[(r-1) * R1 + k] = w_N^(r k N / (R1 R2)),  t3[(r-1) * R1 R2 + k] = w_N^(r k).
+// Costs one LDS.64 per use instead of 2 (R2 - 1 + NB3 (R3 - 1)) registers per thread.
+template <class P>
+struct SmemTwiddles {
+    static constexpr int N2 = (P::R2 > 1 ? P::R2 - 1 : 0) * P::R1;
+    static constexpr int N3 = (P::R3 > 1 ? (P::R3 - 1) * P::R1 * P::R2 : 0);
+    static constexpr int COUNT = N2 + N3;            // float2 entries
+    const float2* t2;
+    const float2* t3;
+    int k2[P::NB2];                                   // (t + T m) mod R1
+    int k3[P::NB3];                                   // (t + T m) mod R1 R2
+
+    // every thread of the CTA calls fill(); the caller synchronises before the first transform
+    __device__ __forceinline__ static void fill(float2* table, const float2* __restrict__ tw, int tid, int nthreads)
+    {
+        for (int i = tid; i < N2; i += nthreads) {
+            const int r = i / P::R1 + 1, k = i % P::R1;
+            table[i] = __ldg(tw + ((r * k * (P::N / (P::R1 * P::R2))) & (P::N - 1)));
+        }
+        for (int i = tid; i < N3; i += nthreads) {
+            const int r = i / (P::R1 * P::R2) + 1, k = i % (P::R1 * P::R2);
+            table[N2 + i] = __ldg(tw + ((r * k) & (P::N - 1)));
+        }
+    }
+    __device__ __forceinline__ void bind(const float2* table, int t)
+    {
+        t2 = table; t3 = table + N2;
+#pragma unroll
+        for (int m = 0; m < P::NB2; ++m) k2[m] = (t + P::T * m) % P::R1;
+#pragma unroll
+        for (int m = 0; m < P::NB3; ++m) k3[m] = (t + P::T * m) % (P::R1 * P::R2);
+    }
+    __device__ __forceinline__ float2 get2(int m, int r) const { return t2[(r - 1) * P::R1 + k2[m]]; }
+    __device__ __forceinline__ float2 get3(int m, int r) const { return t3[(r - 1) * P::R1 * P::R2 + k3[m]]; }
 };
 
 // Shared-memory view of one line's exchange space: element idx lives at
 // base[pad16(idx) * stride].  stride = 1 for a row buffer, (W+1) for a column of
-// a padded [rows][W+1] tile.
+// a padded [rows][W+1] tile.  sync() is a barrier among the threads of one line (or more): the
+// whole warp if the line fits in one, else the whole CTA (every thread of the CTA runs the same sequence).
+template <class P>
 struct LineSmem {
     float2* base;
     int stride;
     __device__ __forceinline__ void  st(int idx, float2 v) const { base[pad16(idx) * stride] = v; }
     __device__ __forceinline__ float2 ld(int idx) const { return base[pad16(idx) * stride]; }
+    __device__ __forceinline__ void sync() const { if (P::T <= 32) __syncwarp(); else __syncthreads(); }
 };
 
-// barrier among the threads of one line (or more): whole warp if the line fits in
-// one, else the whole CTA (every thread of the CTA runs the same sequence).
-template <class P>
-__device__ __forceinline__ void line_sync()
-{
-    if (P::T <= 32) __syncwarp(); else __syncthreads();
-}
-
 // Forward transform of the line held as v[e] = x[t + T e].  Begins with a
-// line_sync(), so `sm` may alias storage the line's threads have just read.
-template <class P>
-__device__ __forceinline__ void fft_forward(float2 (&v)[P::E], const Twiddles<P>& tw, int t, const LineSmem& sm)
+// sm.sync(), so `sm` may alias storage the line's threads have just read.
+// TW supplies get2(m, r) / get3(m, r); SM supplies st(idx, v) / ld(idx) / sync().
+template <class P, class TW, class SM>
+__device__ __forceinline__ void fft_forward(float2 (&v)[P::E], const TW& tw, int t, const SM& sm)
 {
     constexpr int E = P::E, T = P::T;
-    line_sync<P>();                          // earlier readers of `sm` (previous transform, tile loads) are done
+    sm.sync();                               // earlier readers of `sm` (previous transform, tile loads) are done
     // ---- stage 1: radix R1, Ns = 1, no twiddles ----
 #pragma unroll
     for (int m = 0; m < P::NB1; ++m) {
@@ -227,17 +262,17 @@ __device__ __forceinline__ void fft_forward(float2 (&v)[P::E], const Twiddles<P>
 #pragma unroll
         for (int r = 0; r < P::R1; ++r) sm.st(j * P::R1 + r, a[r]);
     }
-    line_sync<P>();
+    sm.sync();
 #pragma unroll
     for (int e = 0; e < E; ++e) v[e] = sm.ld(t + T * e);
     // ---- stage 2: radix R2, Ns = R1 ----
-    if (P::R3 > 1) line_sync<P>();           // all reads done before the next exchange overwrites
+    if (P::R3 > 1) sm.sync();                // all reads done before the next exchange overwrites
 #pragma unroll
     for (int m = 0; m < P::NB2; ++m) {
         float2 a[P::R2];
         a[0] = v[m];
 #pragma unroll
-        for (int r = 1; r < P::R2; ++r) a[r] = cmul(v[m + P::NB2 * r], tw.s2[P::S2_SHARED ? 0 : m][r - 1]);
+        for (int r = 1; r < P::R2; ++r) a[r] = cmul(v[m + P::NB2 * r], tw.get2(m, r));
         Dft<P::R2>::run(a);
         if (P::R3 == 1) {
 #pragma unroll
@@ -251,7 +286,7 @@ __device__ __forceinline__ void fft_forward(float2 (&v)[P::E], const Twiddles<P>
         }
     }
     if (P::R3 > 1) {
-        line_sync<P>();
+        sm.sync();
 #pragma unroll
         for (int e = 0; e < E; ++e) v[e] = sm.ld(t + T * e);
         // ---- stage 3: radix R3, Ns = R1 R2, in place ----
@@ -260,7 +295,7 @@ __device__ __forceinline__ void fft_forward(float2 (&v)[P::E], const Twiddles<P>
             float2 a[P::R3 > 1 ? P::R3 : 1];
             a[0] = v[m];
 #pragma unroll
-            for (int r = 1; r < P::R3; ++r) a[r] = cmul(v[m + P::NB3 * r], tw.s3[m][r - 1]);
+            for (int r = 1; r < P::R3; ++r) a[r] = cmul(v[m + P::NB3 * r], tw.get3(m, r));
             Dft<P::R3>::run(a);
 #pragma unroll
             for (int r = 0; r < P::R3; ++r) v[m + P::NB3 * r] = a[r];
@@ -269,8 +304,8 @@ __device__ __forceinline__ void fft_forward(float2 (&v)[P::E], const Twiddles<P>
 }
 
 // Unscaled inverse transform: forward transform of the (im, re)-swapped data.
-template <class P>
-__device__ __forceinline__ void fft_inverse(float2 (&v)[P::E], const Twiddles<P>& tw, int t, const LineSmem& sm)
+template <class P, class TW, class SM>
+__device__ __forceinline__ void fft_inverse(float2 (&v)[P::E], const TW& tw, int t, const SM& sm)
 {
 #pragma unroll
     for (int e = 0; e < P::E; ++e) v[e] = cswap(v[e]);

@@ -24,9 +24,14 @@ struct RowArgs {
     const float2* tw_y;       // exp(-2 pi i m / ny), m < ny   (ROW_INIT phase of the plane wave)
     const int2*   beams;      // [n_waves] (kx, ky)             (ROW_INIT)
     int           n_waves, nx, ny;
+    int           xband;      // mixed space is read / written for kx in [0, xband) and [nx - xband, nx) only
+                              // (pipelined kernels; everything outside is zero by the 2/3 band-limit)
     float         scale;      // ROW_INIT: plane-wave amplitude; ROW_FINAL: output scale
 };
 cudaError_t launch_row_pass(RowMode mode, const RowArgs& args, cudaStream_t stream);
+// grids whose slice step runs on the pipelined kernels of slice_pipe.cu (both passes or neither)
+inline bool pipelined_grid(int nx, int ny) { return nx >= 256 && ny >= 256; }
+cudaError_t launch_row_pipe(RowMode mode, const RowArgs& args, cudaStream_t stream);
 
 enum ColMode {
     COL_STEP     = 0,   // A -> FFT_y -> * P -> IFFT_y -> A
@@ -47,9 +52,11 @@ struct ColArgs {
     const float2* phase_y;    // [probes_y][ny] exp(-2 pi i ky y_p / ly)
     int           probe0, probes_x;   // wave w is probe probe0 + w; (px, py) = (p % probes_x, p / probes_x)
     int           n_waves, nx, ny;
+    int           xband;      // see RowArgs
     float         scale;      // COL_ABS2 / COL_MS_FINAL intensity scale
 };
 cudaError_t launch_col_pass(ColMode mode, const ColArgs& args, cudaStream_t stream);
+cudaError_t launch_col_pipe(ColMode mode, const ColArgs& args, cudaStream_t stream);
 
 // t = exp(i sigma V) for one slice (Eq. 1), fp64 sincos rounded once to fp32
 cudaError_t launch_transmission(const float* v, float2* t, double sigma, int64_t npix, cudaStream_t stream);

@@ -16,7 +16,7 @@
 namespace prism {
 
 static int g_num_sms = 0;
-static int num_sms()
+int num_sms()
 {
     if (!g_num_sms) {
         int dev = 0;
@@ -45,7 +45,7 @@ __global__ void __launch_bounds__(P::T* LPC) row_pass_kernel(RowArgs g)
     constexpr int E = P::E, T = P::T, N = P::N;
     extern __shared__ float2 smem[];
     const int ll = threadIdx.x / T, t = threadIdx.x % T;
-    LineSmem sm{ smem + ll * P::PADDED, 1 };
+    LineSmem<P> sm{ smem + ll * P::PADDED, 1 };
     Twiddles<P> tw;
     tw.load(g.tw_x, t);
 
@@ -133,6 +133,7 @@ static cudaError_t launch_row_n(RowMode mode, const RowArgs& g, cudaStream_t str
 
 cudaError_t launch_row_pass(RowMode mode, const RowArgs& g, cudaStream_t stream)
 {
+    if (pipelined_grid(g.nx, g.ny) && mode != ROW_FFT) return launch_row_pipe(mode, g, stream);
     switch (g.nx) {
         case 16:   return launch_row_n<16>(mode, g, stream);
         case 32:   return launch_row_n<32>(mode, g, stream);
@@ -183,7 +184,7 @@ __global__ void __launch_bounds__((W / G) * P::T) col_pass_kernel(ColArgs g)
         for (int grp = 0; grp < G; ++grp) {
             const int c = grp * (W / G) + cl;
             const int kxi = kx0 + c;                               // array slot of this column
-            LineSmem sm{ tile + c, CS };
+            LineSmem<P> sm{ tile + c, CS };
             float2 v[E];
 
             if (MODE == COL_MS_INIT) {
@@ -278,6 +279,7 @@ static cudaError_t launch_col_n(ColMode mode, const ColArgs& g, cudaStream_t str
 
 cudaError_t launch_col_pass(ColMode mode, const ColArgs& g, cudaStream_t stream)
 {
+    if (pipelined_grid(g.nx, g.ny) && mode != COL_ABS2) return launch_col_pipe(mode, g, stream);
     if (g.nx % 8 != 0) return cudaErrorInvalidValue;
     switch (g.ny) {
         case 16:   return launch_col_n<16>(mode, g, stream);

@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(_HERE, "libprism_b200.so")
 PRISM_OK, PRISM_EINVAL, PRISM_ENOMEM, PRISM_ECUDA, PRISM_EUNSUPPORTED, PRISM_ENOLUT = 0, -1, -2, -3, -4, -5
 WS_SMATRIX, WS_OUTPUT, WS_MULTISLICE, WS_POTENTIAL = 0, 1, 2, 3
 
-EXPORTS = ["prism_workspace_bytes", "prism_num_bins", "prism_num_beams", "prism_constants",
+EXPORTS = ["prism_workspace_bytes", "prism_num_bins", "prism_num_beams", "prism_band_columns", "prism_constants",
            "prism_build_potential", "prism_compute_smatrix", "prism_compute_output",
            "multislice_compute_output", "prism_strerror", "prism_last_error", "prism_launch_count",
            "prism_timing_enable", "prism_timing_classes", "prism_timing_class_name", "prism_timing_read"]
@@ -61,6 +61,8 @@ def _load() -> C.CDLL:
     lib.prism_workspace_bytes.argtypes = [pp, i32]
     lib.prism_num_bins.restype = i32
     lib.prism_num_bins.argtypes = [pp]
+    lib.prism_band_columns.restype = i32
+    lib.prism_band_columns.argtypes = [pp]
     lib.prism_num_beams.restype = C.c_int
     lib.prism_num_beams.argtypes = [pp, C.POINTER(i32)]
     lib.prism_constants.restype = C.c_int
@@ -132,6 +134,10 @@ def workspace_bytes(p: Params, which: int, n_atoms: int = 0) -> int:
 
 def num_bins(p: Params) -> int:
     return int(_lib.prism_num_bins(C.byref(p)))
+
+
+def band_columns(p: Params) -> int:
+    return int(_lib.prism_band_columns(C.byref(p)))
 
 
 def num_beams(p: Params) -> int:

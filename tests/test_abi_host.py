@@ -68,6 +68,21 @@ def test_beam_counts_and_bins(prism, name, n_beams):
     assert prism.num_bins(p) == O.num_bins(oracle_params(w))
 
 
+@pytest.mark.parametrize("name", ["PR1", "MS2", "P4", "P8"])
+def test_band_columns_cover_the_oracle_propagator(prism, name):
+    """Every kx column in which the oracle's band-limited propagator is non-zero lies inside the column band
+    the library moves through HBM, and the band is not wider than one 32-column rounding."""
+    w = W.get(name)
+    prop = O.propagator(oracle_params(w))
+    live = np.flatnonzero(np.abs(prop).sum(axis=0) > 0)           # kx slots with any non-zero entry
+    c = prism.band_columns(prism.params_from_workload(w))
+    assert c % 32 == 0 and 0 < c <= w.nx // 2
+    inside = (live < c) | (live >= w.nx - c)
+    assert inside.all()
+    kxmax = int(np.max(np.minimum(live, w.nx - live)))
+    assert c == min(w.nx // 2, -(-(kxmax + 1) // 32) * 32)
+
+
 def test_workspace_sizes_are_positive_and_scale(prism):
     w = W.get("P4")
     p = prism.params_from_workload(w)

@@ -142,6 +142,50 @@ def test_prism_output_parity_regular_lattice(G, name):
     assert rel_l2(out[rows], ref2) < 2e-5
 
 
+# ---- large grids: the pipelined slice-step kernels at 1024 and 2048 points per line ---
+def _large_cases():
+    return {
+        # 1024^2 (one-exchange 32 x 32 transform), f=8 -> 128^2 windows, the grid of BASELINE.json config 4
+        "T1024f8": W.scaled_test_case(1024, 3, 8, 4, voltage=200e3, alpha_mrad=12.0, defocus=50.0, seed_index=21,
+                                      density=0.01),
+        # 2048^2 (32 x 16 x 4 transform), f=16 -> 128^2 windows, the grid of config 5; small aperture keeps
+        # the S-matrix of the test at a few GiB
+        "T2048f16": W.scaled_test_case(2048, 2, 16, 4, voltage=300e3, alpha_mrad=6.0, seed_index=22,
+                                       density=0.004),
+    }
+
+
+LARGE = _large_cases()
+
+
+@pytest.mark.parametrize("name", list(LARGE))
+def test_large_grid_parity(G, name):
+    """Oracle by decomposition: sampled S-matrix layers, oracle stage 2 applied to the GPU
+    S-matrix for sampled probes, and sampled multislice probes end to end."""
+    w = LARGE[name]
+    p = oracle_params(w)
+    v = G.gpu_potential(w)
+    v_ref = oracle_potential(w)
+    assert rel_l2(v.cpu().numpy().astype(np.float64), v_ref) < TOL_V
+    s, beams = G.gpu_smatrix(w, v)
+    assert set(map(tuple, beams.tolist())) == set(map(tuple, O.beams(p).tolist()))
+    pick = np.unique(np.linspace(0, len(beams) - 1, 4).astype(int))
+    for b in pick:
+        ref = O.smatrix_layer(p, v_ref, int(beams[b, 0]), int(beams[b, 1]))
+        assert rel_l2(s[b].cpu().numpy().astype(np.complex128), ref) < TOL_S, (name, b)
+    out = G.gpu_prism_output(w, s, beams)
+    xy = w.probe_xy()
+    rows = np.array([0, 5, len(xy) - 1])
+    ref2 = O.prism_probes(p, s.cpu().numpy().astype(np.complex128), beams, xy[rows])
+    assert rel_l2(out[rows], ref2) < 2e-5
+    del s
+    ms = G.gpu_multislice(w, v)
+    ref3 = O.multislice_probes(p, v_ref, xy[rows])
+    assert rel_l2(ms[rows], ref3) < TOL_OUT
+    d = G.dark_field(w, p)
+    assert rel_l2(ms[rows][:, d:], ref3[:, d:]) < 5 * TOL_OUT
+
+
 def test_lattice_path_does_not_depend_on_batch(G):
     from paper_1706_08563_b200 import prism
     w = LATTICE["L128f2part"]
