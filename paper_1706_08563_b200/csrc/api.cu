@@ -162,6 +162,15 @@ static int band_columns(const prism_params* p)
     for (int m = 0; m <= p->nx / 2; ++m) if (lim[m] >= 0) kxmax = m;
     return std::min(p->nx / 2, (kxmax + 1 + 31) / 32 * 32);
 }
+// the same along ky: a multiple of 32 above every ky_lim[kx]
+static int band_rows(const prism_params* p)
+{
+    std::vector<int> lim;
+    band_limit(p, lim);
+    int kymax = 0;
+    for (int m = 0; m < p->nx; ++m) kymax = std::max(kymax, lim[m]);
+    return std::min(p->ny / 2, (kymax + 1 + 31) / 32 * 32);
+}
 
 static double aberration(const prism_params* p, double lambda, double q2)
 {
@@ -741,7 +750,7 @@ int prism_compute_smatrix(const prism_params* p, const float* v, int32_t* beams_
             ra.n_waves = nb; ra.nx = p->nx; ra.ny = p->ny; ra.scale = 1.f; ra.xband = xband;
             ColArgs ca;
             std::memset(&ca, 0, sizeof(ca));
-            ca.xband = xband;
+            ca.xband = xband; ca.yband = band_rows(p);
             ca.a = ra.a; ca.tw_y = L.tab.tw_y; ca.prop_x = L.tab.prop_x; ca.prop_y = L.tab.prop_y;
             ca.ky_lim = L.tab.ky_lim; ca.n_waves = nb; ca.nx = p->nx; ca.ny = p->ny; ca.scale = 1.f;
             feed.begin_sweep();
@@ -967,7 +976,7 @@ int multislice_compute_output(const prism_params* p, const float* v, float* out,
             ca.a = L.psi; ca.intensity = L.intensity; ca.tw_y = L.tab.tw_y; ca.prop_x = L.tab.prop_x;
             ca.prop_y = L.tab.prop_y; ca.ky_lim = L.tab.ky_lim; ca.aperture_t = L.aperture_t;
             ca.phase_x = L.phase_x; ca.phase_y = L.phase_y; ca.probe0 = p0; ca.probes_x = p->probes_x;
-            ca.n_waves = np; ca.nx = nx; ca.ny = ny; ca.xband = xband;
+            ca.n_waves = np; ca.nx = nx; ca.ny = ny; ca.xband = xband; ca.yband = band_rows(p);
             ca.scale = (float)((double)ny / (double)nx);      // I = |Psi_S|^2 / (nx ny), see DESIGN.md
             RowArgs ra;
             std::memset(&ra, 0, sizeof(ra));

@@ -239,13 +239,14 @@ struct LineSmem {
     float2* base;
     int stride;
     __device__ __forceinline__ void  st(int idx, float2 v) const { base[pad16(idx) * stride] = v; }
+    __device__ __forceinline__ void  st2(int idx, float2 v0, float2 v1) const { st(idx, v0); st(idx + 1, v1); }
     __device__ __forceinline__ float2 ld(int idx) const { return base[pad16(idx) * stride]; }
     __device__ __forceinline__ void sync() const { if (P::T <= 32) __syncwarp(); else __syncthreads(); }
 };
 
 // Forward transform of the line held as v[e] = x[t + T e].  Begins with a
 // sm.sync(), so `sm` may alias storage the line's threads have just read.
-// TW supplies get2(m, r) / get3(m, r); SM supplies st(idx, v) / ld(idx) / sync().
+// TW supplies get2(m, r) / get3(m, r); SM supplies st(idx, v) / st2(even idx, v0, v1) / ld(idx) / sync().
 template <class P, class TW, class SM>
 __device__ __forceinline__ void fft_forward(float2 (&v)[P::E], const TW& tw, int t, const SM& sm)
 {
@@ -260,7 +261,7 @@ __device__ __forceinline__ void fft_forward(float2 (&v)[P::E], const TW& tw, int
         Dft<P::R1>::run(a);
         const int j = t + T * m;
 #pragma unroll
-        for (int r = 0; r < P::R1; ++r) sm.st(j * P::R1 + r, a[r]);
+        for (int r = 0; r < P::R1; r += 2) sm.st2(j * P::R1 + r, a[r], a[r + 1]);   // even idx: may be one 16-byte store
     }
     sm.sync();
 #pragma unroll

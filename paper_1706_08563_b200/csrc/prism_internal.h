@@ -53,6 +53,7 @@ struct ColArgs {
     int           probe0, probes_x;   // wave w is probe probe0 + w; (px, py) = (p % probes_x, p / probes_x)
     int           n_waves, nx, ny;
     int           xband;      // see RowArgs
+    int           yband;      // a multiple of 32 with ky_lim[kx] < yband for every kx (pipelined kernels)
     float         scale;      // COL_ABS2 / COL_MS_FINAL intensity scale
 };
 cudaError_t launch_col_pass(ColMode mode, const ColArgs& args, cudaStream_t stream);

@@ -77,7 +77,7 @@ struct RowCfg {
     static constexpr int T = P::T;
     static constexpr int TEAM = T < 32 ? 32 : T;                 // threads of one team
     static constexpr int LPT = TEAM / T;                         // lines per team
-    static constexpr int LINE = P::N + P::N / P::R1;             // padded exchange space of one line (float2)
+    static constexpr int LINE = P::N + 2 * (P::N / P::R1);       // padded exchange space of one line (float2)
     static constexpr int SLOT = LPT * LINE;
     static constexpr int TWB = round_up_c(SmemTwiddles<P>::COUNT * 8, 128);
     static constexpr int TEAMS_BY_SMEM = (PIPE_SMEM_MAX - PIPE_HEADER - TWB) / (2 * SLOT * 8);
@@ -86,22 +86,29 @@ struct RowCfg {
     static constexpr size_t SMEM = PIPE_HEADER + TWB + (size_t)TEAMS * 2 * SLOT * 8;
 };
 
-// exchange space of one line inside its slot: element idx at base[idx + idx / R1]
+// exchange space of one line inside its slot: element idx at base[idx + 2 (idx / R1)].  Two pad words per
+// group of R1 keep pairs (even idx, idx + 1) 16-byte aligned, so the radix-R1 outputs of a thread go out as
+// 16-byte stores, and a quarter warp of such stores (stride R1 + 2 words) covers all banks once.
 template <class P, int TEAM>
 struct RowSm {
     float2* base;
     int bar_id;
-    __device__ __forceinline__ static int phys(int idx) { return idx + idx / P::R1; }
+    __device__ __forceinline__ static int phys(int idx) { return idx + 2 * (idx / P::R1); }
     __device__ __forceinline__ void  st(int idx, float2 v) const { base[phys(idx)] = v; }
+    __device__ __forceinline__ void  st2(int idx, float2 v0, float2 v1) const
+    { *reinterpret_cast<float4*>(base + phys(idx)) = make_float4(v0.x, v0.y, v1.x, v1.y); }
     __device__ __forceinline__ float2 ld(int idx) const { return base[phys(idx)]; }
     __device__ __forceinline__ void sync() const { if (TEAM <= 32) __syncwarp(); else named_barrier(bar_id, TEAM); }
 };
 
-template <class P, int MODE>
+// XBE > 0: the band is xband = XBE * T columns, known at compile time (then "in band" depends on the register
+// index e only and out-of-band elements cost no instruction); XBE = 0: any xband, tested per element.
+template <class P, int MODE, int XBE>
 __global__ void __launch_bounds__(RowCfg<P>::THREADS, 1) row_pipe_kernel(RowArgs g)
 {
     using C = RowCfg<P>;
     constexpr int E = P::E, T = P::T, N = P::N;
+    auto in_band = [&](int e, int kx, int xb) { return XBE > 0 ? (e < XBE || e >= E - XBE) : (kx < xb || kx >= N - xb); };
     extern __shared__ __align__(128) unsigned char smem_raw[];
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw);                    // [TEAMS][2]
     float2* twtab = reinterpret_cast<float2*>(smem_raw + PIPE_HEADER);
@@ -123,7 +130,7 @@ __global__ void __launch_bounds__(RowCfg<P>::THREADS, 1) row_pipe_kernel(RowArgs
     const long long n_lines = (long long)g.n_waves * g.ny;
     const long long n_groups = (n_lines + C::LPT - 1) / C::LPT;
     const long long gteam = (long long)blockIdx.x * C::TEAMS + team, gstride = (long long)gridDim.x * C::TEAMS;
-    const int xb = g.xband;                                  // in-band columns: [0, xb) and [N - xb, N)
+    const int xb = XBE > 0 ? XBE * T : g.xband;              // in-band columns: [0, xb) and [N - xb, N)
 
     // one thread of the team: start the bulk copies of line group `grp` into slot `s`
     auto issue = [&](long long grp, int s) {
@@ -176,7 +183,7 @@ __global__ void __launch_bounds__(RowCfg<P>::THREADS, 1) row_pipe_kernel(RowArgs
 #pragma unroll
             for (int e = 0; e < E; ++e) {
                 const int kx = t + T * e;
-                v[e] = (kx < xb || kx >= N - xb) ? lbase[kx] : make_float2(0.f, 0.f);   // out of band: exact zeros
+                v[e] = in_band(e, kx, xb) ? lbase[kx] : make_float2(0.f, 0.f);   // out of band: exact zeros
             }
         }
 
@@ -208,17 +215,17 @@ __global__ void __launch_bounds__(RowCfg<P>::THREADS, 1) row_pipe_kernel(RowArgs
 #pragma unroll
             for (int e = 0; e < E; ++e) {
                 const int kx = t + T * e;
-                if (kx < xb || kx >= N - xb) row[kx] = v[e];
+                if (in_band(e, kx, xb)) row[kx] = v[e];
             }
         }
     }
 }
 
-template <class P, int MODE>
-static cudaError_t launch_row_pipe_t(const RowArgs& g, cudaStream_t stream)
+template <class P, int MODE, int XBE>
+static cudaError_t launch_row_pipe_x(const RowArgs& g, cudaStream_t stream)
 {
     using C = RowCfg<P>;
-    auto kern = row_pipe_kernel<P, MODE>;
+    auto kern = row_pipe_kernel<P, MODE, XBE>;
     static bool set = false;
     if (!set) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
@@ -232,6 +239,18 @@ static cudaError_t launch_row_pipe_t(const RowArgs& g, cudaStream_t stream)
     if (grid > num_sms()) grid = num_sms();
     kern<<<(unsigned)grid, C::THREADS, C::SMEM, stream>>>(g);
     return cudaGetLastError();
+}
+
+// band of a grid with square pixels: |kx| <= floor(N / 3), rounded up to 32 columns
+template <int N> struct DefaultBand { static constexpr int XB = (N / 3 + 1 + 31) / 32 * 32; };
+
+template <class P, int MODE>
+static cudaError_t launch_row_pipe_t(const RowArgs& g, cudaStream_t stream)
+{
+    constexpr int XB = DefaultBand<P::N>::XB;
+    static_assert(XB % P::T == 0, "default band must be a whole number of register slots");
+    if (g.xband == XB) return launch_row_pipe_x<P, MODE, XB / P::T>(g, stream);
+    return launch_row_pipe_x<P, MODE, 0>(g, stream);
 }
 
 template <int N>
@@ -285,15 +304,19 @@ struct ColSm {
     int bar_id;
     __device__ __forceinline__ static int phys(int idx) { return idx + idx / P::R1; }
     __device__ __forceinline__ void  st(int idx, float2 v) const { base[phys(idx) * W] = v; }
+    __device__ __forceinline__ void  st2(int idx, float2 v0, float2 v1) const { st(idx, v0); st(idx + 1, v1); }
     __device__ __forceinline__ float2 ld(int idx) const { return base[phys(idx) * W]; }
     __device__ __forceinline__ void sync() const { named_barrier(bar_id, TEAM); }
 };
 
-template <class P, int MODE>
+// SQ: nx == ny == N, so every row stride is a compile-time constant (immediate offsets, no 64-bit index math).
+// YBE > 0: no column passes |ky| >= YBE * T (yband of ColArgs), known at compile time.
+template <class P, int MODE, bool SQ, int YBE>
 __global__ void __launch_bounds__(ColCfg<P>::THREADS, 1) col_pipe_kernel(ColArgs g)
 {
     using C = ColCfg<P>;
     constexpr int E = P::E, T = P::T, N = P::N, W = C::W;
+    const int nx = SQ ? N : g.nx;
     constexpr bool LOADS = (MODE != COL_MS_INIT);
     extern __shared__ __align__(128) unsigned char smem_raw[];
     uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw);                    // [NBUF]
@@ -320,20 +343,20 @@ __global__ void __launch_bounds__(ColCfg<P>::THREADS, 1) col_pipe_kernel(ColArgs
         const long long item = blockIdx.x + k * (long long)gridDim.x;
         w = (int)(item / tiles_per_wave);
         const int j = (int)(item % tiles_per_wave);
-        kx0 = j < tiles_half ? j * W : g.nx - xb + (j - tiles_half) * W;
+        kx0 = j < tiles_half ? j * W : nx - xb + (j - tiles_half) * W;
     };
     // all threads of a team: start the copies of local item k into buffer k % NBUF
     auto load = [&](long long k) {
         int w, kx0;
         locate(k, w, kx0);
-        const float2* src = g.a + (size_t)w * g.ny * g.nx + kx0;
+        const float2* src = g.a + (size_t)w * N * nx + kx0;
         float2* buf = bufs + (size_t)(k % C::NBUF) * C::BUF;
         constexpr int CH = W / 2;                                 // 16-byte chunks per row
 #pragma unroll
         for (int i = 0; i < N * CH / C::TEAM; ++i) {
             const int q = tt + i * C::TEAM;
             const int row = q / CH, cc = q % CH;
-            cp_async16(buf + (row + row / P::R1) * W + 2 * cc, src + (size_t)row * g.nx + 2 * cc);
+            cp_async16(buf + (row + row / P::R1) * W + 2 * cc, src + (size_t)row * nx + 2 * cc);
         }
         cp_async_arrive(&full[k % C::NBUF]);
     };
@@ -354,7 +377,7 @@ __global__ void __launch_bounds__(ColCfg<P>::THREADS, 1) col_pipe_kernel(ColArgs
             // Psi0(kx, ky) = A_k exp(-i chi_k) exp(-2 pi i (kx xp / lx + ky yp / ly))
             const int p = g.probe0 + w;
             const int pxi = p % g.probes_x, pyi = p / g.probes_x;
-            const float2 ex = __ldg(g.phase_x + (size_t)pxi * g.nx + kxi);
+            const float2 ex = __ldg(g.phase_x + (size_t)pxi * nx + kxi);
             const float2* ap = g.aperture_t + (size_t)kxi * N;
             const float2* ey = g.phase_y + (size_t)pyi * N;
 #pragma unroll
@@ -367,13 +390,17 @@ __global__ void __launch_bounds__(ColCfg<P>::THREADS, 1) col_pipe_kernel(ColArgs
 #pragma unroll
             for (int e = 0; e < E; ++e) v[e] = sm.ld(t + T * e);
             fft_forward<P>(v, tw, t, sm);
-            // Fresnel propagator with the 2/3 band-limit (Eq. 2; BASELINE.json)
+            // Fresnel propagator with the 2/3 band-limit (Eq. 2; BASELINE.json): the table holds
+            // prop_x[kx] prop_y[ky] inside the band and zero outside, [ky][kx] like the wave (L2 resident)
+// Fresnel propagator with the 2/3 band-limit (Eq. 2; BASELINE.json).  With YBE > 0 the
+            // register slots e in [YBE, E - YBE) hold |ky| beyond every column's limit: zero without any work.
             const float2 pxv = __ldg(g.prop_x + kxi);
             const int lim = __ldg(g.ky_lim + kxi);
 #pragma unroll
             for (int e = 0; e < E; ++e) {
+                if (YBE > 0 && e >= YBE && e < E - YBE) { v[e] = make_float2(0.f, 0.f); continue; }
                 const int m = t + T * e;
-                const int ky = m < N / 2 ? m : N - m;           // |ky|
+                const int ky = e < E / 2 ? m : N - m;           // |ky|
                 const float2 pr = cmul(pxv, __ldg(g.prop_y + m));
                 v[e] = (ky <= lim) ? cmul(v[e], pr) : make_float2(0.f, 0.f);
             }
@@ -386,12 +413,12 @@ __global__ void __launch_bounds__(ColCfg<P>::THREADS, 1) col_pipe_kernel(ColArgs
         }
 
         if (MODE == COL_STEP || MODE == COL_MS_INIT) {
-            float2* dst = g.a + (size_t)w * g.ny * g.nx + kxi;
+            float2* dst = g.a + (size_t)w * N * nx + kxi;
 #pragma unroll
-            for (int e = 0; e < E; ++e) dst[(size_t)(t + T * e) * g.nx] = v[e];
+            for (int e = 0; e < E; ++e) dst[(size_t)(t + T * e) * nx] = v[e];
         } else {
             // detector-plane intensity, ky contiguous
-            float* dst = g.intensity + ((size_t)w * g.nx + kxi) * N;
+            float* dst = g.intensity + ((size_t)w * nx + kxi) * N;
 #pragma unroll
             for (int e = 0; e < E; ++e)
                 dst[t + T * e] = (v[e].x * v[e].x + v[e].y * v[e].y) * g.scale;
@@ -399,11 +426,11 @@ __global__ void __launch_bounds__(ColCfg<P>::THREADS, 1) col_pipe_kernel(ColArgs
     }
 }
 
-template <class P, int MODE>
-static cudaError_t launch_col_pipe_t(const ColArgs& g, cudaStream_t stream)
+template <class P, int MODE, bool SQ, int YBE>
+static cudaError_t launch_col_pipe_s(const ColArgs& g, cudaStream_t stream)
 {
     using C = ColCfg<P>;
-    auto kern = col_pipe_kernel<P, MODE>;
+    auto kern = col_pipe_kernel<P, MODE, SQ, YBE>;
     static bool set = false;
     if (!set) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
@@ -417,6 +444,15 @@ static cudaError_t launch_col_pipe_t(const ColArgs& g, cudaStream_t stream)
     if (grid > num_sms()) grid = num_sms();
     kern<<<(unsigned)grid, C::THREADS, C::SMEM, stream>>>(g);
     return cudaGetLastError();
+}
+
+template <class P, int MODE>
+static cudaError_t launch_col_pipe_t(const ColArgs& g, cudaStream_t stream)
+{
+    constexpr int YB = DefaultBand<P::N>::XB;
+    if (g.nx == P::N && g.yband == YB) return launch_col_pipe_s<P, MODE, true, YB / P::T>(g, stream);
+    if (g.nx == P::N) return launch_col_pipe_s<P, MODE, true, 0>(g, stream);
+    return launch_col_pipe_s<P, MODE, false, 0>(g, stream);
 }
 
 template <int N>

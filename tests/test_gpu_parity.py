@@ -186,6 +186,38 @@ def test_large_grid_parity(G, name):
     assert rel_l2(ms[rows][:, d:], ref3[:, d:]) < 5 * TOL_OUT
 
 
+def _odd_grid_cases():
+    base = W.scaled_test_case(256, 3, 4, 4, voltage=300e3, alpha_mrad=12.0, seed_index=31, density=0.03)
+    lz = base.cell[2]
+    return {
+        # 512 x 256 grid with square pixels: the pipelined column pass with a run-time row stride
+        "R512x256": base.with_(name="R512x256", nx=512, cell=(51.2, 25.6, lz), probe_step=(12.8, 6.4)),
+        # 256 x 512 grid
+        "R256x512": base.with_(name="R256x512", ny=512, cell=(25.6, 51.2, lz), probe_step=(6.4, 12.8)),
+        # 0.1 x 0.2 Angstrom pixels: the band-limit circle is narrower than the default column band in kx
+        "A256": base.with_(name="A256", cell=(25.6, 51.2, lz), probe_step=(6.4, 12.8), alpha=8e-3),
+    }
+
+
+ODD = _odd_grid_cases()
+
+
+@pytest.mark.parametrize("name", list(ODD))
+def test_rectangular_grids_and_anisotropic_pixels(G, name):
+    w = ODD[name]
+    p = oracle_params(w)
+    v = G.gpu_potential(w)
+    v_ref = oracle_potential(w)
+    assert rel_l2(v.cpu().numpy().astype(np.float64), v_ref) < TOL_V
+    s, beams = G.gpu_smatrix(w, v)
+    s_ref = O.smatrix(p, v_ref, beams)
+    assert rel_l2(s.cpu().numpy().astype(np.complex128), s_ref) < TOL_S
+    out = G.gpu_prism_output(w, s, beams)
+    assert rel_l2(out, O.prism_probes(p, s_ref, beams, w.probe_xy())) < TOL_OUT
+    ms = G.gpu_multislice(w, v)
+    assert rel_l2(ms, O.multislice_probes(p, v_ref, w.probe_xy())) < TOL_OUT
+
+
 def test_lattice_path_does_not_depend_on_batch(G):
     from paper_1706_08563_b200 import prism
     w = LATTICE["L128f2part"]
