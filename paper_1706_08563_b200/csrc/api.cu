@@ -262,6 +262,7 @@ struct SliceFeeder {
     int64_t npix = 0;
     int n_slices = 0;
     double sigma = 0;
+    bool pairs = false;                 // transmission function in pair layout (packed row pass)
     float2* tbuf = nullptr;
     float* ring[RING] = {nullptr, nullptr, nullptr};
     cudaStream_t main_stream = nullptr, copy_stream = nullptr;
@@ -309,7 +310,7 @@ struct SliceFeeder {
             CU(cudaStreamWaitEvent(main_stream, filled[r], 0));
             src = ring[r];
         }
-        LAUNCH(K_TRANSMISSION, launch_transmission(src, tbuf, sigma, npix, main_stream), main_stream);
+        LAUNCH(K_TRANSMISSION, launch_transmission(src, tbuf, sigma, npix, pairs, main_stream), main_stream);
         if (on_host) CU(cudaEventRecord(consumed[s % RING], main_stream));
         return PRISM_OK;
     }
@@ -736,7 +737,7 @@ int prism_compute_smatrix(const prism_params* p, const float* v, int32_t* beams_
     const size_t npix = (size_t)p->nx * p->ny;
     SliceFeeder& feed = L.feed;
     feed.v = v; feed.on_host = p->potential_on_host != 0; feed.npix = (int64_t)npix; feed.n_slices = p->n_slices;
-    feed.sigma = sigma; feed.main_stream = st;
+    feed.sigma = sigma; feed.main_stream = st; feed.pairs = packed_row(p->nx, p->ny);
     if ((rc = feed.init())) { feed.release(); return rc; }
 
     const int batch = p->batch > 0 ? std::min<int>(p->batch, n_beams) : n_beams;
@@ -960,7 +961,7 @@ int multislice_compute_output(const prism_params* p, const float* v, float* out,
 
     SliceFeeder& feed = L.feed;
     feed.v = v; feed.on_host = p->potential_on_host != 0; feed.npix = (int64_t)npix; feed.n_slices = p->n_slices;
-    feed.sigma = sigma; feed.main_stream = st;
+    feed.sigma = sigma; feed.main_stream = st; feed.pairs = packed_row(p->nx, p->ny);
     if ((rc = feed.init())) { feed.release(); return rc; }
 
     const int n_probes = p->probes_x * p->probes_y;

@@ -23,8 +23,14 @@
 
 namespace prism {
 
+#ifndef PRISM_PACKED_ADDS
 __device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
 __device__ __forceinline__ float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
+#else
+// sm_100a packed fp32: one FADD2 per complex add (same rounding as two FADDs, half the issue slots)
+__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return __fadd2_rn(a, b); }
+__device__ __forceinline__ float2 csub(float2 a, float2 b) { return __fadd2_rn(a, make_float2(-b.x, -b.y)); }
+#endif
 __device__ __forceinline__ float2 cmul(float2 a, float2 b)
 { return make_float2(fmaf(a.x, b.x, -a.y * b.y), fmaf(a.x, b.y, a.y * b.x)); }
 __device__ __forceinline__ float2 cmul_conj(float2 a, float2 b)   // a * conj(b)

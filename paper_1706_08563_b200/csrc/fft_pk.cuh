@@ -1,0 +1,277 @@
+// fft_pk.cuh -- two-way packed complex64 line FFT for sm_100a (FADD2 / FMUL2 / FFMA2).
+//
+// Blackwell's packed fp32 instructions do two fp32 operations per issue slot (same lane throughput as
+// the scalar forms, half the instructions).  A line of N points is split by one radix-2 step into two
+// independent half-length transforms with identical structure and twiddles (even / odd outputs for
+// decimation in frequency, even / odd inputs for decimation in time); the two halves travel through
+// the radix-32 register butterflies as the two lanes of every packed operation:
+//
+//   C2 { x = (re_a, re_b), y = (im_a, im_b) }         a, b = the two half-length transforms
+//
+// so one instruction stream of a half-length FFT transforms the whole line, and each exchange through
+// shared memory moves a 16-byte (a, b) pair per access.  A line is held by T = N / 64 threads with 64
+// points each: 32 packed pairs in the half transforms, 64 scalar complex values at the radix-2 step.
+//
+//   layout L1 ("natural"): v[e]  = x[t + T e],               e  < 64  (8-byte coalesced access)
+//   layout L2 ("paired") : p[e]  = (x[2 j], x[2 j + 1]), j = t + T e, e < 32
+//
+//   forward DIF : L1 in  -> L2 out        forward DIT : L2 in -> L1 out
+//   inverse     : the forward transform on (im, re)-swapped data (a register renaming)
+//
+// The half-length transform is H = N / 2 = 32 x R2 points (R2 = 4 .. 32): one radix-32 butterfly per
+// thread, ONE exchange, NB2 = 32 / R2 radix-R2 butterflies.  Twiddles are fp64-built table values.
+//
+// Implements the transforms of PAPER.md:80 (Eq. 2: FFT / inverse FFT around the propagator).
+#pragma once
+#include <cuda_runtime.h>
+
+namespace prism {
+namespace pk {
+
+struct C2 { float2 x, y; };      // x: real parts of (a, b); y: imaginary parts of (a, b)
+
+__device__ __forceinline__ float2 neg2(float2 a) { return make_float2(-a.x, -a.y); }
+__device__ __forceinline__ float2 add2(float2 a, float2 b) { return __fadd2_rn(a, b); }
+__device__ __forceinline__ float2 sub2(float2 a, float2 b) { return __fadd2_rn(a, neg2(b)); }
+__device__ __forceinline__ float2 mul2(float2 a, float2 b) { return __fmul2_rn(a, b); }
+__device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c) { return __ffma2_rn(a, b, c); }
+__device__ __forceinline__ float2 bc(float c) { return make_float2(c, c); }
+
+__device__ __forceinline__ C2 cadd(C2 a, C2 b) { return { add2(a.x, b.x), add2(a.y, b.y) }; }
+__device__ __forceinline__ C2 csub(C2 a, C2 b) { return { sub2(a.x, b.x), sub2(a.y, b.y) }; }
+__device__ __forceinline__ C2 cadd_mi(C2 a, C2 b) { return { add2(a.x, b.y), sub2(a.y, b.x) }; }   // a + (-i) b
+__device__ __forceinline__ C2 csub_mi(C2 a, C2 b) { return { sub2(a.x, b.y), add2(a.y, b.x) }; }   // a - (-i) b
+__device__ __forceinline__ C2 cswap(C2 a) { return { a.y, a.x }; }
+// a * (wr + i wi), the same factor for both lanes
+__device__ __forceinline__ C2 cmulc(C2 a, float wr, float wi)
+{
+    return { fma2(a.x, bc(wr), mul2(a.y, bc(-wi))), fma2(a.x, bc(wi), mul2(a.y, bc(wr))) };
+}
+// a * w with separate factors for the two lanes: wr = (wr_a, wr_b), wi = (wi_a, wi_b)
+__device__ __forceinline__ C2 cmul2(C2 a, float2 wr, float2 wi)
+{
+    return { fma2(a.x, wr, neg2(mul2(a.y, wi))), fma2(a.x, wi, mul2(a.y, wr)) };
+}
+
+template <int R> struct Dft;
+
+template <> struct Dft<1> { __device__ __forceinline__ static void run(C2*) {} };
+
+template <> struct Dft<2> {
+    __device__ __forceinline__ static void run(C2* a)
+    { C2 t = a[0]; a[0] = cadd(t, a[1]); a[1] = csub(t, a[1]); }
+};
+
+template <> struct Dft<4> {
+    __device__ __forceinline__ static void run(C2* a)
+    {
+        const C2 t0 = cadd(a[0], a[2]), t1 = csub(a[0], a[2]);
+        const C2 t2 = cadd(a[1], a[3]), d = csub(a[1], a[3]);
+        a[0] = cadd(t0, t2); a[2] = csub(t0, t2);
+        a[1] = cadd_mi(t1, d); a[3] = csub_mi(t1, d);
+    }
+};
+
+template <> struct Dft<8> {
+    __device__ __forceinline__ static void run(C2* a)
+    {
+        const float h = 0.70710678118654752440f;
+        C2 e[4] = { a[0], a[2], a[4], a[6] };
+        C2 o[4] = { a[1], a[3], a[5], a[7] };
+        Dft<4>::run(e); Dft<4>::run(o);
+        a[0] = cadd(e[0], o[0]); a[4] = csub(e[0], o[0]);
+        {   // o1 * w8, w8 = (1 - i) / sqrt2 :  (h (x + y), h (y - x))
+            const float2 p = add2(o[1].x, o[1].y), q = sub2(o[1].y, o[1].x);
+            a[1] = { fma2(p, bc(h), e[1].x), fma2(q, bc(h), e[1].y) };
+            a[5] = { fma2(p, bc(-h), e[1].x), fma2(q, bc(-h), e[1].y) };
+        }
+        a[2] = cadd_mi(e[2], o[2]); a[6] = csub_mi(e[2], o[2]);
+        {   // o3 * w8^3 = (-1 - i) / sqrt2 :  (h (y - x), -h (x + y))
+            const float2 p = add2(o[3].x, o[3].y), q = sub2(o[3].y, o[3].x);
+            a[3] = { fma2(q, bc(h), e[3].x), fma2(p, bc(-h), e[3].y) };
+            a[7] = { fma2(q, bc(-h), e[3].x), fma2(p, bc(h), e[3].y) };
+        }
+    }
+};
+
+template <> struct Dft<16> {
+    __device__ __forceinline__ static void run(C2* a)
+    {
+        const float c1 = 0.92387953251128675613f, s1 = 0.38268343236508977173f;   // cos, sin(pi/8)
+        const float h  = 0.70710678118654752440f;
+        C2 y[4][4];
+#pragma unroll
+        for (int n2 = 0; n2 < 4; ++n2) {
+            y[n2][0] = a[n2]; y[n2][1] = a[n2 + 4]; y[n2][2] = a[n2 + 8]; y[n2][3] = a[n2 + 12];
+            Dft<4>::run(y[n2]);
+        }
+        // w16^m = exp(-2 pi i m / 16)
+        y[1][1] = cmulc(y[1][1], c1, -s1);
+        y[1][2] = cmulc(y[1][2], h, -h);
+        y[1][3] = cmulc(y[1][3], s1, -c1);
+        y[2][1] = cmulc(y[2][1], h, -h);
+        y[2][2] = { y[2][2].y, neg2(y[2][2].x) };
+        y[2][3] = cmulc(y[2][3], -h, -h);
+        y[3][1] = cmulc(y[3][1], s1, -c1);
+        y[3][2] = cmulc(y[3][2], -h, -h);
+        y[3][3] = cmulc(y[3][3], -c1, s1);
+#pragma unroll
+        for (int k1 = 0; k1 < 4; ++k1) {
+            C2 z[4] = { y[0][k1], y[1][k1], y[2][k1], y[3][k1] };
+            Dft<4>::run(z);
+            a[k1] = z[0]; a[k1 + 4] = z[1]; a[k1 + 8] = z[2]; a[k1 + 12] = z[3];
+        }
+    }
+};
+
+template <> struct Dft<32> {
+    __device__ __forceinline__ static void run(C2* a)
+    {
+        // n = 4 n1 + n2 (n1 < 8, n2 < 4); k = k1 + 8 k2.  Y[n2][k1] = DFT8 over n1, twiddle w32^(n2 k1), DFT4 over n2.
+        // w32^m = exp(-2 pi i m / 32) = (WC[m], -WS[m]) for m <= 21
+        constexpr float WC[22] = { 1.f, 0.98078528040323044913f, 0.92387953251128675613f, 0.83146961230254523708f,
+                                   0.70710678118654752440f, 0.55557023301960222474f, 0.38268343236508977173f,
+                                   0.19509032201612826785f, 0.f, -0.19509032201612826785f, -0.38268343236508977173f,
+                                   -0.55557023301960222474f, -0.70710678118654752440f, -0.83146961230254523708f,
+                                   -0.92387953251128675613f, -0.98078528040323044913f, -1.f, -0.98078528040323044913f,
+                                   -0.92387953251128675613f, -0.83146961230254523708f, -0.70710678118654752440f,
+                                   -0.55557023301960222474f };
+        constexpr float WS[22] = { 0.f, 0.19509032201612826785f, 0.38268343236508977173f, 0.55557023301960222474f,
+                                   0.70710678118654752440f, 0.83146961230254523708f, 0.92387953251128675613f,
+                                   0.98078528040323044913f, 1.f, 0.98078528040323044913f, 0.92387953251128675613f,
+                                   0.83146961230254523708f, 0.70710678118654752440f, 0.55557023301960222474f,
+                                   0.38268343236508977173f, 0.19509032201612826785f, 0.f, -0.19509032201612826785f,
+                                   -0.38268343236508977173f, -0.55557023301960222474f, -0.70710678118654752440f,
+                                   -0.83146961230254523708f };
+        C2 y[4][8];
+#pragma unroll
+        for (int n2 = 0; n2 < 4; ++n2) {
+#pragma unroll
+            for (int n1 = 0; n1 < 8; ++n1) y[n2][n1] = a[4 * n1 + n2];
+            Dft<8>::run(y[n2]);
+        }
+#pragma unroll
+        for (int n2 = 1; n2 < 4; ++n2)
+#pragma unroll
+            for (int k1 = 1; k1 < 8; ++k1) {
+                if (n2 * k1 == 8) y[n2][k1] = { y[n2][k1].y, neg2(y[n2][k1].x) };      // * (-i)
+                else y[n2][k1] = cmulc(y[n2][k1], WC[n2 * k1], -WS[n2 * k1]);
+            }
+#pragma unroll
+        for (int k1 = 0; k1 < 8; ++k1) {
+            C2 z[4] = { y[0][k1], y[1][k1], y[2][k1], y[3][k1] };
+            Dft<4>::run(z);
+            a[k1] = z[0]; a[k1 + 8] = z[1]; a[k1 + 16] = z[2]; a[k1 + 24] = z[3];
+        }
+    }
+};
+
+// ---- half-length transform: H = 32 x R2 points by T = H / 32 threads, 32 packed pairs per thread ------
+template <int N_>
+struct PkPlan {
+    static constexpr int N = N_, H = N_ / 2, T = N_ / 64, R1 = 32, R2 = H / 32, NB2 = 32 / R2;
+    static_assert(N_ >= 256 && N_ <= 2048 && (N_ & (N_ - 1)) == 0, "line length");
+    static constexpr int XPAD = H + H / 32;                 // exchange space of one line, in C2 (16-byte) units
+    static constexpr int TW2 = (R2 - 1) * 32;               // stage-2 twiddles w_H^(r k), float2 each
+    static constexpr int TWN = H;                           // radix-2 twiddles w_N^n, n < N / 2
+    static constexpr int TW_BYTES = (TW2 + TWN) * 8;
+};
+
+// tables in shared memory: t2[(r - 1) * 32 + k] = w_H^(r k) (k < 32, r < R2), tn[n] = w_N^n (n < N / 2);
+// tw_n is the caller's table exp(-2 pi i m / N), m < N.  Every thread of the CTA calls fill().
+template <class P>
+__device__ __forceinline__ void fill_tables(float2* table, const float2* __restrict__ tw_n, int tid, int nthreads)
+{
+    for (int i = tid; i < P::TW2; i += nthreads) {
+        const int r = i / 32 + 1, k = i % 32;
+        table[i] = __ldg(tw_n + ((2 * r * k) & (P::N - 1)));          // w_H^(r k) = w_N^(2 r k)
+    }
+    for (int i = tid; i < P::TWN; i += nthreads) table[P::TW2 + i] = __ldg(tw_n + i);
+}
+
+// exchange space view: element idx (a 16-byte pair) at base[(idx + idx / 32) * stride]
+struct Xchg {
+    float4* base;
+    int stride;
+    __device__ __forceinline__ void st(int idx, C2 v) const
+    { base[(idx + (idx >> 5)) * stride] = make_float4(v.x.x, v.x.y, v.y.x, v.y.y); }
+    __device__ __forceinline__ C2 ld(int idx) const
+    { const float4 q = base[(idx + (idx >> 5)) * stride]; return { make_float2(q.x, q.y), make_float2(q.z, q.w) }; }
+};
+
+// Forward half-length transforms of both lanes: p[e] holds element t + T e (layout in = layout out).
+// SYNC() is a barrier among (at least) the threads of the line; the function begins with one, so the
+// exchange space may alias storage those threads have just read.
+template <class P, class SYNC>
+__device__ __forceinline__ void fft_half(C2 (&p)[32], const float2* __restrict__ t2, int t, const Xchg& sm, SYNC sync)
+{
+    constexpr int T = P::T;
+    sync();
+    Dft<32>::run(p);
+#pragma unroll
+    for (int r = 0; r < 32; ++r) sm.st(t * 32 + r, p[r]);
+    sync();
+#pragma unroll
+    for (int e = 0; e < 32; ++e) p[e] = sm.ld(t + T * e);
+#pragma unroll
+    for (int m = 0; m < P::NB2; ++m) {
+        C2 a[P::R2];
+        const int k = (t + T * m) & 31;
+        a[0] = p[m];
+#pragma unroll
+        for (int r = 1; r < P::R2; ++r) {
+            const float2 w = t2[(r - 1) * 32 + k];
+            a[r] = cmulc(p[m + P::NB2 * r], w.x, w.y);
+        }
+        Dft<P::R2>::run(a);
+#pragma unroll
+        for (int r = 0; r < P::R2; ++r) p[m + P::NB2 * r] = a[r];
+    }
+}
+
+// Band description of a length-N axis in layout L1: slot e (element t + T e) is kept iff e < XBE or e >= 64 - XBE.
+// XBE = 32 keeps everything.
+template <int XBE> __device__ __forceinline__ constexpr bool kept(int e) { return e < XBE || e >= 64 - XBE; }
+
+// Forward DIF: v (L1; slots not kept<IN>() are taken as exact zeros) -> p (L2 pairs).
+template <class P, int IN, class SYNC>
+__device__ __forceinline__ void fft_dif(const float2 (&v)[64], C2 (&p)[32], const float2* __restrict__ tab, int t,
+                                        const Xchg& sm, SYNC sync)
+{
+    const float2* tn = tab + P::TW2;
+#pragma unroll
+    for (int e = 0; e < 32; ++e) {
+        const float2 w = tn[t + P::T * e];                       // w_N^n, n = t + T e
+        float2 a, d;
+        if (kept<IN>(e) && kept<IN>(e + 32)) {
+            a = make_float2(v[e].x + v[e + 32].x, v[e].y + v[e + 32].y);
+            d = make_float2(v[e].x - v[e + 32].x, v[e].y - v[e + 32].y);
+        } else if (kept<IN>(e)) { a = v[e]; d = v[e]; }
+        else if (kept<IN>(e + 32)) { a = v[e + 32]; d = make_float2(-v[e + 32].x, -v[e + 32].y); }
+        else { a = make_float2(0.f, 0.f); d = a; }
+        const float2 b = make_float2(fmaf(d.x, w.x, -d.y * w.y), fmaf(d.x, w.y, d.y * w.x));
+        p[e] = { make_float2(a.x, b.x), make_float2(a.y, b.y) };
+    }
+    fft_half<P>(p, tab, t, sm, sync);
+}
+
+// Forward DIT: p (L2 pairs) -> v (L1); only slots kept<OUT>() are computed.
+template <class P, int OUT, class SYNC>
+__device__ __forceinline__ void fft_dit(C2 (&p)[32], float2 (&v)[64], const float2* __restrict__ tab, int t,
+                                        const Xchg& sm, SYNC sync)
+{
+    fft_half<P>(p, tab, t, sm, sync);
+    const float2* tn = tab + P::TW2;
+#pragma unroll
+    for (int e = 0; e < 32; ++e) {
+        if (!kept<OUT>(e) && !kept<OUT>(e + 32)) continue;
+        const float2 w = tn[t + P::T * e];                       // w_N^k, k = t + T e
+        const float2 a = make_float2(p[e].x.x, p[e].y.x), b = make_float2(p[e].x.y, p[e].y.y);
+        const float2 bw = make_float2(fmaf(b.x, w.x, -b.y * w.y), fmaf(b.x, w.y, b.y * w.x));
+        if (kept<OUT>(e)) v[e] = make_float2(a.x + bw.x, a.y + bw.y);
+        if (kept<OUT>(e + 32)) v[e + 32] = make_float2(a.x - bw.x, a.y - bw.y);
+    }
+}
+
+}  // namespace pk
+}  // namespace prism

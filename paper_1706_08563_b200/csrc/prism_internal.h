@@ -32,6 +32,10 @@ cudaError_t launch_row_pass(RowMode mode, const RowArgs& args, cudaStream_t stre
 // grids whose slice step runs on the pipelined kernels of slice_pipe.cu (both passes or neither)
 inline bool pipelined_grid(int nx, int ny) { return nx >= 256 && ny >= 256; }
 cudaError_t launch_row_pipe(RowMode mode, const RowArgs& args, cudaStream_t stream);
+// line lengths whose row pass runs on the packed-FFT kernels of slice_pk.cu; their transmission function is
+// stored in pair layout t[y][j] = (re(2j), re(2j+1), im(2j), im(2j+1))
+inline bool packed_row(int nx, int ny) { return pipelined_grid(nx, ny) && nx == 2048; }
+cudaError_t launch_row_pk(RowMode mode, const RowArgs& args, cudaStream_t stream);
 
 enum ColMode {
     COL_STEP     = 0,   // A -> FFT_y -> * P -> IFFT_y -> A
@@ -58,9 +62,12 @@ struct ColArgs {
 };
 cudaError_t launch_col_pass(ColMode mode, const ColArgs& args, cudaStream_t stream);
 cudaError_t launch_col_pipe(ColMode mode, const ColArgs& args, cudaStream_t stream);
+// column lengths whose column pass runs on the packed-FFT kernels of slice_pk.cu
+inline bool packed_col(int nx, int ny) { return pipelined_grid(nx, ny) && ny == 2048; }
+cudaError_t launch_col_pk(ColMode mode, const ColArgs& args, cudaStream_t stream);
 
 // t = exp(i sigma V) for one slice (Eq. 1), fp64 sincos rounded once to fp32
-cudaError_t launch_transmission(const float* v, float2* t, double sigma, int64_t npix, cudaStream_t stream);
+cudaError_t launch_transmission(const float* v, float2* t, double sigma, int64_t npix, bool pairs, cudaStream_t stream);
 
 // ---- stage 2 (output.cu) ---------------------------------------------------------
 struct BeamSumArgs {

@@ -133,6 +133,7 @@ static cudaError_t launch_row_n(RowMode mode, const RowArgs& g, cudaStream_t str
 
 cudaError_t launch_row_pass(RowMode mode, const RowArgs& g, cudaStream_t stream)
 {
+    if (packed_row(g.nx, g.ny) && mode != ROW_FFT) return launch_row_pk(mode, g, stream);
     if (pipelined_grid(g.nx, g.ny) && mode != ROW_FFT) return launch_row_pipe(mode, g, stream);
     switch (g.nx) {
         case 16:   return launch_row_n<16>(mode, g, stream);
@@ -279,6 +280,7 @@ static cudaError_t launch_col_n(ColMode mode, const ColArgs& g, cudaStream_t str
 
 cudaError_t launch_col_pass(ColMode mode, const ColArgs& g, cudaStream_t stream)
 {
+    if (packed_col(g.nx, g.ny) && mode != COL_ABS2) return launch_col_pk(mode, g, stream);
     if (pipelined_grid(g.nx, g.ny) && mode != COL_ABS2) return launch_col_pipe(mode, g, stream);
     if (g.nx % 8 != 0) return cudaErrorInvalidValue;
     switch (g.ny) {
@@ -298,25 +300,38 @@ cudaError_t launch_col_pass(ColMode mode, const ColArgs& g, cudaStream_t stream)
 // Transmission function of one slice, Eq. (1): t = exp(i sigma V).
 // Computed once per slice (not per wave) in fp64 and rounded once to fp32.
 // =============================================================================
+// PAIRS: pixels (2j, 2j+1) are stored as (re, re, im, im), the layout the packed row pass multiplies in.
+template <bool PAIRS>
 __global__ void transmission_kernel(const float* __restrict__ v, float2* __restrict__ t, double sigma, int64_t npix)
 {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
-    for (; i < npix; i += stride) {
-        double s, c;
-        sincos(sigma * (double)v[i], &s, &c);
-        t[i] = make_float2((float)c, (float)s);
+    if (PAIRS) {
+        for (; i < npix / 2; i += stride) {
+            const float2 vv = reinterpret_cast<const float2*>(v)[i];
+            double s0, c0, s1, c1;
+            sincos(sigma * (double)vv.x, &s0, &c0);
+            sincos(sigma * (double)vv.y, &s1, &c1);
+            reinterpret_cast<float4*>(t)[i] = make_float4((float)c0, (float)c1, (float)s0, (float)s1);
+        }
+    } else {
+        for (; i < npix; i += stride) {
+            double s, c;
+            sincos(sigma * (double)v[i], &s, &c);
+            t[i] = make_float2((float)c, (float)s);
+        }
     }
 }
 
-cudaError_t launch_transmission(const float* v, float2* t, double sigma, int64_t npix, cudaStream_t stream)
+cudaError_t launch_transmission(const float* v, float2* t, double sigma, int64_t npix, bool pairs, cudaStream_t stream)
 {
     if (npix == 0) return cudaSuccess;
     const int threads = 256;
     long long blocks = (npix + threads - 1) / threads;
     const long long cap = (long long)num_sms() * 8;
     if (blocks > cap) blocks = cap;
-    transmission_kernel<<<(unsigned)blocks, threads, 0, stream>>>(v, t, sigma, npix);
+    if (pairs) transmission_kernel<true><<<(unsigned)blocks, threads, 0, stream>>>(v, t, sigma, npix);
+    else transmission_kernel<false><<<(unsigned)blocks, threads, 0, stream>>>(v, t, sigma, npix);
     return cudaGetLastError();
 }
 

@@ -1,0 +1,420 @@
+// slice_pk.cu -- slice-step passes on the two-way packed FFT of fft_pk.cuh (FADD2 / FMUL2 / FFMA2).
+//
+// PAPER.md:44 Eq. (1)  psi <- psi * exp(i sigma V)          (transmission)
+// PAPER.md:80 Eq. (2)  Psi <- Psi * exp(-i pi lambda q^2 t)  (propagation), "done in Fourier space"
+//
+// Same two passes, same mixed-space storage A[w][y][kx] and the same band-limit bookkeeping as
+// slice_pipe.cu; what changes is the transform: a line of N points is held by N / 64 threads (64 points
+// each), split by one radix-2 step in registers into two half-length transforms that run as the two
+// lanes of packed fp32 instructions, so a transform needs ONE shared-memory exchange up to 2048 points,
+// only warp-level barriers in the row pass, and about half the instructions per point:
+//
+//   row pass    : A (natural kx) -> inverse DIF -> real space in pairs (x[2j], x[2j+1]) -> * t_s (stored in
+//                 the same pair layout by the transmission kernel) -> forward DIT -> A (natural kx)
+//   column pass : A (natural y) -> forward DIF -> pairs (ky = 2j, 2j+1) -> * P -> inverse DIT -> A (natural y)
+//
+// so global memory is always read and written in natural order with coalesced accesses and no register
+// shuffling is needed between the pair layout and memory.
+#include "fft_core.cuh"
+#include "fft_pk.cuh"
+#include "pipe_ptx.cuh"
+#include "prism_internal.h"
+
+namespace prism {
+
+using pk::C2;
+
+// =============================================================================
+// Row pass
+// =============================================================================
+// XBE < 32: the band is xband = XBE * T columns, known at compile time; XBE = 32: any xband, tested per element.
+template <int N, int XBE>
+struct RowPkCfg {
+    using P = pk::PkPlan<N>;
+    static constexpr int T = P::T, LPW = 32 / T;                   // threads per line, lines per warp
+    static constexpr int LANDW = XBE < 32 ? 2 * XBE * T : N;       // points of a line that are moved
+    static constexpr int LAND_BYTES = LPW * LANDW * 8;
+    static constexpr int X_BYTES = LPW * P::XPAD * 16;
+    static constexpr int PER_WARP = LAND_BYTES + X_BYTES;
+    static constexpr int TWB = round_up_c(P::TW_BYTES, 128);
+    static constexpr int BY_SMEM = (PIPE_SMEM_MAX - PIPE_HEADER - TWB) / PER_WARP;
+    static constexpr int WARPS = BY_SMEM < 8 ? BY_SMEM : 8;
+    static constexpr int THREADS = WARPS * 32;
+    static constexpr size_t SMEM = PIPE_HEADER + TWB + (size_t)WARPS * PER_WARP;
+};
+
+template <int N, int MODE, int XBE>
+__global__ void __launch_bounds__(RowPkCfg<N, XBE>::THREADS, 1) row_pk_kernel(RowArgs g)
+{
+    using C = RowPkCfg<N, XBE>;
+    using P = typename C::P;
+    constexpr int T = P::T, LPW = C::LPW;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw);                    // [WARPS]
+    float2* tab = reinterpret_cast<float2*>(smem_raw + PIPE_HEADER);
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int ll = lane / T, t = lane % T;
+    unsigned char* mine = smem_raw + PIPE_HEADER + C::TWB + (size_t)warp * C::PER_WARP;
+    float2* land = reinterpret_cast<float2*>(mine);                            // [LPW][LANDW]
+    float4* xch = reinterpret_cast<float4*>(mine + C::LAND_BYTES);             // [LPW][XPAD]
+
+    pk::fill_tables<P>(tab, g.tw_x, tid, C::THREADS);
+    if (MODE != ROW_INIT && lane == 0) { mbar_init(&bars[warp], 1); mbar_fence_init(); }
+    __syncthreads();
+
+    const long long n_lines = (long long)g.n_waves * g.ny;
+    const long long n_groups = (n_lines + LPW - 1) / LPW;
+    const long long gw = (long long)blockIdx.x * C::WARPS + warp, gstride = (long long)gridDim.x * C::WARPS;
+    const int xb = XBE < 32 ? XBE * T : g.xband;                 // in-band columns: [0, xb) and [N - xb, N)
+
+    // lane 0: start the bulk copies of line group `grp` into the landing buffer
+    auto issue = [&](long long grp) {
+        int n_act = 0;
+#pragma unroll
+        for (int l = 0; l < LPW; ++l) n_act += (grp * LPW + l < n_lines);
+        mbar_expect_tx(&bars[warp], (unsigned)(n_act * 2 * xb * (int)sizeof(float2)));
+#pragma unroll
+        for (int l = 0; l < LPW; ++l) {
+            const long long line = grp * LPW + l;
+            if (line < n_lines) {
+                const int y = (int)(line / g.n_waves), w = (int)(line % g.n_waves);
+                const float2* row = g.a + ((size_t)w * g.ny + y) * N;
+                float2* dst = land + l * C::LANDW;
+                bulk_g2s(dst, row, (unsigned)(xb * sizeof(float2)), &bars[warp]);
+                bulk_g2s(dst + xb, row + (N - xb), (unsigned)(xb * sizeof(float2)), &bars[warp]);
+            }
+        }
+    };
+    if (MODE != ROW_INIT && lane == 0 && gw < n_groups) issue(gw);
+
+    const pk::Xchg sm{ xch + ll * P::XPAD, 1 };
+    auto sync = [] { __syncwarp(); };
+    auto in_band = [&](int e) { return XBE < 32 ? pk::kept<XBE>(e) : (t + T * e < xb || t + T * e >= N - xb); };
+
+    int it = 0;
+    for (long long grp = gw; grp < n_groups; grp += gstride, ++it) {
+        long long line = grp * LPW + ll;
+        const bool active = line < n_lines;
+        if (!active) line = n_lines - 1;                 // keep every lane in the warp barriers
+        const int y = (int)(line / g.n_waves), w = (int)(line % g.n_waves);
+        float2* row = g.a + ((size_t)w * g.ny + y) * N;
+        C2 p[32];
+
+        if (MODE == ROW_INIT) {
+            // plane wave exp(+2 pi i (kx x / nx + ky y / ny)) * amplitude at x = 2 j, 2 j + 1
+            const int2 b = g.beams[w];
+            const float2 wy = __ldg(g.tw_y + ((b.y * y) & (g.ny - 1)));
+            const float2 base = make_float2(wy.x * g.scale, -wy.y * g.scale);
+#pragma unroll
+            for (int e = 0; e < 32; ++e) {
+                const int x0 = 2 * (t + T * e);
+                const float2 w0 = __ldg(g.tw_x + ((b.x * x0) & (N - 1)));
+                const float2 w1 = __ldg(g.tw_x + ((b.x * (x0 + 1)) & (N - 1)));
+                const float2 v0 = cmul_conj(base, w0), v1 = cmul_conj(base, w1);
+                p[e] = { make_float2(v0.x, v1.x), make_float2(v0.y, v1.y) };
+            }
+        } else {
+            float2 v[64];
+            mbar_wait(&bars[warp], (unsigned)(it & 1));
+            const float2* lbase = land + ll * C::LANDW;
+#pragma unroll
+            for (int e = 0; e < 64; ++e) {
+                const int kx = t + T * e;
+                int pos;                                    // compact landing: [0, xb) then [N - xb, N)
+                if (XBE < 32) pos = e < XBE ? kx : kx - (N - 2 * xb);
+                else pos = kx < xb ? kx : (kx >= N - xb ? kx - (N - 2 * xb) : 0);
+                if (XBE < 32 && !pk::kept<XBE>(e)) { v[e] = make_float2(0.f, 0.f); continue; }
+                const float2 q = lbase[pos];
+                v[e] = in_band(e) ? make_float2(q.y, q.x) : make_float2(0.f, 0.f);   // (im, re): inverse = swapped forward
+            }
+            // the landing buffer is free once every lane has read its points
+            __syncwarp();
+            if (lane == 0 && grp + gstride < n_groups) { fence_proxy_async(); issue(grp + gstride); }
+            pk::fft_dif<P, XBE>(v, p, tab, t, sm, sync);
+#pragma unroll
+            for (int e = 0; e < 32; ++e) p[e] = pk::cswap(p[e]);
+        }
+
+        if (MODE == ROW_INIT || MODE == ROW_STEP) {
+            // transmission function in pair layout: (re(2j), re(2j+1), im(2j), im(2j+1))
+            const float4* trow = reinterpret_cast<const float4*>(g.t) + (size_t)y * (N / 2);
+#pragma unroll
+            for (int e = 0; e < 32; ++e) {
+                const float4 q = __ldg(trow + t + T * e);
+                p[e] = pk::cmul2(p[e], make_float2(q.x, q.y), make_float2(q.z, q.w));
+            }
+        }
+
+        if (MODE == ROW_FINAL) {
+            float4* dst = reinterpret_cast<float4*>(g.out + ((size_t)w * g.ny + y) * N);
+            if (active) {
+#pragma unroll
+                for (int e = 0; e < 32; ++e)
+                    dst[t + T * e] = make_float4(p[e].x.x * g.scale, p[e].y.x * g.scale, p[e].x.y * g.scale, p[e].y.y * g.scale);
+            }
+        } else {
+            float2 v[64];
+            pk::fft_dit<P, XBE>(p, v, tab, t, sm, sync);
+            if (active) {
+#pragma unroll
+                for (int e = 0; e < 64; ++e)
+                    if (in_band(e)) row[t + T * e] = v[e];
+            }
+        }
+    }
+}
+
+template <int N, int MODE, int XBE>
+static cudaError_t launch_row_pk_x(const RowArgs& g, cudaStream_t stream)
+{
+    using C = RowPkCfg<N, XBE>;
+    auto kern = row_pk_kernel<N, MODE, XBE>;
+    static bool set = false;
+    if (!set) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
+        if (e != cudaSuccess) return e;
+        set = true;
+    }
+    const long long n_lines = (long long)g.n_waves * g.ny;
+    const long long n_groups = (n_lines + C::LPW - 1) / C::LPW;
+    if (n_groups == 0) return cudaSuccess;
+    long long grid = (n_groups + C::WARPS - 1) / C::WARPS;
+    if (grid > num_sms()) grid = num_sms();
+    kern<<<(unsigned)grid, C::THREADS, C::SMEM, stream>>>(g);
+    return cudaGetLastError();
+}
+
+template <int N, int MODE>
+static cudaError_t launch_row_pk_t(const RowArgs& g, cudaStream_t stream)
+{
+    constexpr int XB = DefaultBand<N>::XB, T = N / 64;
+    static_assert(XB % T == 0, "default band must be a whole number of register slots");
+    if (g.xband == XB) return launch_row_pk_x<N, MODE, XB / T>(g, stream);
+    return launch_row_pk_x<N, MODE, 32>(g, stream);
+}
+
+template <int N>
+static cudaError_t launch_row_pk_n(RowMode mode, const RowArgs& g, cudaStream_t stream)
+{
+    switch (mode) {
+        case ROW_INIT:  return launch_row_pk_t<N, ROW_INIT>(g, stream);
+        case ROW_STEP:  return launch_row_pk_t<N, ROW_STEP>(g, stream);
+        case ROW_FINAL: return launch_row_pk_t<N, ROW_FINAL>(g, stream);
+        default: break;
+    }
+    return cudaErrorInvalidValue;
+}
+
+cudaError_t launch_row_pk(RowMode mode, const RowArgs& g, cudaStream_t stream)
+{
+    if (g.xband < 32 || g.xband % 32 || 2 * g.xband > g.nx) return cudaErrorInvalidValue;
+    switch (g.nx) {
+        case 1024: return launch_row_pk_n<1024>(mode, g, stream);
+        case 2048: return launch_row_pk_n<2048>(mode, g, stream);
+    }
+    return cudaErrorInvalidValue;
+}
+
+// =============================================================================
+// Column pass
+// =============================================================================
+template <int N>
+struct ColPkCfg {
+    using P = pk::PkPlan<N>;
+    static constexpr int T = P::T;
+    static constexpr int TILE_PTS = 8192;
+    static constexpr int W = TILE_PTS / N;                       // columns per tile: 8 (1024), 4 (2048)
+    static constexpr int TEAM = W * T;                           // 128 threads per team
+    static constexpr int LPW = 32 / W;                           // threads of one column inside a warp
+    static constexpr int BUF_BYTES = P::XPAD * W * 16;           // a tile buffer doubles as the exchange space
+    static constexpr int NBUF = 3;
+    static constexpr int THREADS = 2 * TEAM;
+    static constexpr int TWB = round_up_c(P::TW_BYTES, 128);
+    static constexpr size_t SMEM = PIPE_HEADER + TWB + (size_t)NBUF * BUF_BYTES;
+    static_assert((TEAM / 32) * LPW == T, "team shape");
+    static_assert(SMEM <= PIPE_SMEM_MAX, "tile ring does not fit");
+};
+
+// SQ: nx == ny == N (compile-time row stride).  YBE > 0: no column passes |ky| >= 2 T YBE (yband of ColArgs),
+// known at compile time: the pair slots e in [YBE, 32 - YBE) are zero after the propagator.
+template <int N, int MODE, bool SQ, int YBE>
+__global__ void __launch_bounds__(ColPkCfg<N>::THREADS, 1) col_pk_kernel(ColArgs g)
+{
+    using C = ColPkCfg<N>;
+    using P = typename C::P;
+    constexpr int T = P::T, W = C::W;
+    const int nx = SQ ? N : g.nx;
+    constexpr bool LOADS = (MODE != COL_MS_INIT);
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw);                    // [NBUF]
+    float2* tab = reinterpret_cast<float2*>(smem_raw + PIPE_HEADER);
+    unsigned char* bufs = smem_raw + PIPE_HEADER + C::TWB;
+    const int tid = threadIdx.x, tm = tid / C::TEAM, tt = tid % C::TEAM;
+    const int lane = tt & 31, c = lane % W, t = (tt >> 5) * C::LPW + lane / W;
+
+    pk::fill_tables<P>(tab, g.tw_y, tid, C::THREADS);
+    if (LOADS && tid == 0) {
+        for (int b = 0; b < C::NBUF; ++b) mbar_init(&full[b], C::TEAM);
+        mbar_fence_init();
+    }
+    __syncthreads();
+
+    const int xb = g.xband;
+    const int tiles_half = xb / W, tiles_per_wave = 2 * tiles_half;
+    const long long n_items = (long long)g.n_waves * tiles_per_wave;
+    const long long n_local = (n_items > blockIdx.x) ? (n_items - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
+    auto locate = [&](long long k, int& w, int& kx0) {
+        const long long item = blockIdx.x + k * (long long)gridDim.x;
+        w = (int)(item / tiles_per_wave);
+        const int j = (int)(item % tiles_per_wave);
+        kx0 = j < tiles_half ? j * W : nx - xb + (j - tiles_half) * W;
+    };
+    // all threads of a team: start the copies of local item k into buffer k % NBUF (rows in natural order)
+    auto load = [&](long long k) {
+        int w, kx0;
+        locate(k, w, kx0);
+        const float2* src = g.a + (size_t)w * N * nx + kx0;
+        float2* buf = reinterpret_cast<float2*>(bufs + (size_t)(k % C::NBUF) * C::BUF_BYTES);
+        constexpr int CH = W / 2;                                 // 16-byte chunks per row
+#pragma unroll
+        for (int i = 0; i < N * CH / C::TEAM; ++i) {
+            const int q = tt + i * C::TEAM;
+            const int row = q / CH, cc = q % CH;
+            cp_async16(buf + row * W + 2 * cc, src + (size_t)row * nx + 2 * cc);
+        }
+        cp_async_arrive(&full[k % C::NBUF]);
+    };
+    if (LOADS) {
+        if (tm == 0) { if (n_local > 0) load(0); if (n_local > 2) load(2); }
+        else         { if (n_local > 1) load(1); }
+    }
+    auto sync = [&] { named_barrier(1 + tm, C::TEAM); };
+
+    for (long long k = tm; k < n_local; k += 2) {
+        int w, kx0;
+        locate(k, w, kx0);
+        const int kxi = kx0 + c;                                   // array slot of this thread's column
+        const int bi = LOADS ? (int)(k % C::NBUF) : tm;
+        unsigned char* buf = bufs + (size_t)bi * C::BUF_BYTES;
+        const pk::Xchg sm{ reinterpret_cast<float4*>(buf) + c, W };
+        C2 p[32];
+
+        if (MODE == COL_MS_INIT) {
+            // Psi0(kx, ky) = A_k exp(-i chi_k) exp(-2 pi i (kx xp / lx + ky yp / ly)) at ky = 2 j, 2 j + 1
+            const int pr = g.probe0 + w;
+            const int pxi = pr % g.probes_x, pyi = pr / g.probes_x;
+            const float2 ex = __ldg(g.phase_x + (size_t)pxi * nx + kxi);
+            const float4* ap = reinterpret_cast<const float4*>(g.aperture_t + (size_t)kxi * N);
+            const float4* ey = reinterpret_cast<const float4*>(g.phase_y + (size_t)pyi * N);
+#pragma unroll
+            for (int e = 0; e < 32; ++e) {
+                const int j = t + T * e;
+                const float4 a = __ldg(ap + j), y = __ldg(ey + j);
+                const float2 v0 = cmul(cmul(make_float2(a.x, a.y), ex), make_float2(y.x, y.y));
+                const float2 v1 = cmul(cmul(make_float2(a.z, a.w), ex), make_float2(y.z, y.w));
+                p[e] = { make_float2(v0.y, v1.y), make_float2(v0.x, v1.x) };       // (im, re): inverse = swapped forward
+            }
+        } else {
+            float2 v[64];
+            mbar_wait(&full[bi], (unsigned)((k / C::NBUF) & 1));
+            const float2* tile = reinterpret_cast<const float2*>(buf) + c;
+#pragma unroll
+            for (int e = 0; e < 64; ++e) v[e] = tile[(t + T * e) * W];
+            pk::fft_dif<P, 32>(v, p, tab, t, sm, sync);
+            // Fresnel propagator with the 2/3 band-limit (Eq. 2; BASELINE.json) at ky = 2 j, 2 j + 1
+            const float2 pxv = __ldg(g.prop_x + kxi);
+            const int lim = __ldg(g.ky_lim + kxi);
+            const float4* py4 = reinterpret_cast<const float4*>(g.prop_y);
+#pragma unroll
+            for (int e = 0; e < 32; ++e) {
+                if (YBE > 0 && e >= YBE && e < 32 - YBE) { p[e] = { make_float2(0.f, 0.f), make_float2(0.f, 0.f) }; continue; }
+                const int m0 = 2 * (t + T * e);
+                const int ky0 = e < 16 ? m0 : N - m0, ky1 = e < 16 ? m0 + 1 : N - m0 - 1;     // |ky|
+                const float4 q = __ldg(py4 + t + T * e);
+                float2 pr0 = cmul(pxv, make_float2(q.x, q.y)), pr1 = cmul(pxv, make_float2(q.z, q.w));
+                if (ky0 > lim) pr0 = make_float2(0.f, 0.f);
+                if (ky1 > lim) pr1 = make_float2(0.f, 0.f);
+                p[e] = pk::cmul2(p[e], make_float2(pr0.x, pr1.x), make_float2(pr0.y, pr1.y));
+                if (MODE == COL_STEP) p[e] = pk::cswap(p[e]);
+            }
+        }
+
+        if (MODE == COL_STEP || MODE == COL_MS_INIT) {
+            float2 v[64];
+            pk::fft_dit<P, 32>(p, v, tab, t, sm, sync);
+            if (LOADS && k + C::NBUF < n_local) {
+                sync();                              // every thread of the team is past its last exchange read
+                load(k + C::NBUF);
+            }
+            float2* dst = g.a + (size_t)w * N * nx + kxi;
+#pragma unroll
+            for (int e = 0; e < 64; ++e) dst[(size_t)(t + T * e) * nx] = make_float2(v[e].y, v[e].x);
+        } else {
+            if (k + C::NBUF < n_local) {
+                sync();
+                load(k + C::NBUF);
+            }
+            // detector-plane intensity, ky contiguous
+            float2* dst = reinterpret_cast<float2*>(g.intensity + ((size_t)w * nx + kxi) * N);
+#pragma unroll
+            for (int e = 0; e < 32; ++e) {
+                const float2 i2 = pk::fma2(p[e].x, p[e].x, pk::mul2(p[e].y, p[e].y));
+                dst[t + T * e] = make_float2(i2.x * g.scale, i2.y * g.scale);
+            }
+        }
+    }
+}
+
+template <int N, int MODE, bool SQ, int YBE>
+static cudaError_t launch_col_pk_s(const ColArgs& g, cudaStream_t stream)
+{
+    using C = ColPkCfg<N>;
+    auto kern = col_pk_kernel<N, MODE, SQ, YBE>;
+    static bool set = false;
+    if (!set) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
+        if (e != cudaSuccess) return e;
+        set = true;
+    }
+    if (g.xband % C::W || g.nx % C::W) return cudaErrorInvalidValue;
+    const long long n_items = (long long)g.n_waves * (2 * g.xband / C::W);
+    if (n_items == 0) return cudaSuccess;
+    long long grid = (n_items + 1) / 2;                             // at least one tile per team
+    if (grid > num_sms()) grid = num_sms();
+    kern<<<(unsigned)grid, C::THREADS, C::SMEM, stream>>>(g);
+    return cudaGetLastError();
+}
+
+template <int N, int MODE>
+static cudaError_t launch_col_pk_t(const ColArgs& g, cudaStream_t stream)
+{
+    constexpr int YB = DefaultBand<N>::XB, T = N / 64;
+    static_assert(YB % (2 * T) == 0, "default band must be a whole number of pair slots");
+    if (g.nx == N && g.yband == YB) return launch_col_pk_s<N, MODE, true, YB / (2 * T)>(g, stream);
+    if (g.nx == N) return launch_col_pk_s<N, MODE, true, 0>(g, stream);
+    return launch_col_pk_s<N, MODE, false, 0>(g, stream);
+}
+
+template <int N>
+static cudaError_t launch_col_pk_n(ColMode mode, const ColArgs& g, cudaStream_t stream)
+{
+    switch (mode) {
+        case COL_STEP:     return launch_col_pk_t<N, COL_STEP>(g, stream);
+        case COL_MS_INIT:  return launch_col_pk_t<N, COL_MS_INIT>(g, stream);
+        case COL_MS_FINAL: return launch_col_pk_t<N, COL_MS_FINAL>(g, stream);
+        default: break;
+    }
+    return cudaErrorInvalidValue;
+}
+
+cudaError_t launch_col_pk(ColMode mode, const ColArgs& g, cudaStream_t stream)
+{
+    if (g.xband < 4 || 2 * g.xband > g.nx) return cudaErrorInvalidValue;
+    switch (g.ny) {
+        case 1024: return launch_col_pk_n<1024>(mode, g, stream);
+        case 2048: return launch_col_pk_n<2048>(mode, g, stream);
+    }
+    return cudaErrorInvalidValue;
+}
+
+}  // namespace prism
