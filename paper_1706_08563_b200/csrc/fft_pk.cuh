@@ -189,8 +189,10 @@ __device__ __forceinline__ void fill_tables(float2* table, const float2* __restr
     for (int i = tid; i < P::TWN; i += nthreads) table[P::TW2 + i] = __ldg(tw_n + i);
 }
 
-// exchange space view: element idx (a 16-byte pair) at base[(idx + idx / 32) * stride]
-struct Xchg {
+// Exchange space views.  Element idx is an (a, b) pair of complex values.
+// Xchg16: one 16-byte word (re_a, re_b, im_a, im_b) at base[(idx + idx / 32) * stride].
+struct Xchg16 {
+    static constexpr bool TWO_PHASE = false;
     float4* base;
     int stride;
     __device__ __forceinline__ void st(int idx, C2 v) const
@@ -198,21 +200,57 @@ struct Xchg {
     __device__ __forceinline__ C2 ld(int idx) const
     { const float4 q = base[(idx + (idx >> 5)) * stride]; return { make_float2(q.x, q.y), make_float2(q.z, q.w) }; }
 };
+// Xchg8: two 8-byte words, the real parts at base[(idx + idx / 32) * stride] and the imaginary parts `plane`
+// words further on (keeps the packed register pairs free of 16-byte alignment constraints: fewer MOVs, twice
+// the shared-memory instructions).
+struct Xchg8 {
+    static constexpr bool TWO_PHASE = false;
+    float2* base;
+    int stride, plane;
+    __device__ __forceinline__ void st(int idx, C2 v) const
+    { float2* q = base + (idx + (idx >> 5)) * stride; q[0] = v.x; q[plane] = v.y; }
+    __device__ __forceinline__ C2 ld(int idx) const
+    { const float2* q = base + (idx + (idx >> 5)) * stride; return { q[0], q[plane] }; }
+};
+
+// XchgPhase: one 8-byte plane used twice -- real parts first, imaginary parts after a barrier (half the space,
+// two more barriers per transform; the row pass uses it to fit one more warp per SM).
+struct XchgPhase {
+    static constexpr bool TWO_PHASE = true;
+    float2* base;
+    int stride;
+    __device__ __forceinline__ void st(int idx, float2 v) const { base[(idx + (idx >> 5)) * stride] = v; }
+    __device__ __forceinline__ float2 ld(int idx) const { return base[(idx + (idx >> 5)) * stride]; }
+};
 
 // Forward half-length transforms of both lanes: p[e] holds element t + T e (layout in = layout out).
 // SYNC() is a barrier among (at least) the threads of the line; the function begins with one, so the
 // exchange space may alias storage those threads have just read.
-template <class P, class SYNC>
-__device__ __forceinline__ void fft_half(C2 (&p)[32], const float2* __restrict__ t2, int t, const Xchg& sm, SYNC sync)
+template <class P, class SM, class SYNC>
+__device__ __forceinline__ void fft_half(C2 (&p)[32], const float2* __restrict__ t2, int t, const SM& sm, SYNC sync)
 {
     constexpr int T = P::T;
     sync();
     Dft<32>::run(p);
+    if constexpr (SM::TWO_PHASE) {
 #pragma unroll
-    for (int r = 0; r < 32; ++r) sm.st(t * 32 + r, p[r]);
-    sync();
+        for (int r = 0; r < 32; ++r) sm.st(t * 32 + r, p[r].x);
+        sync();
 #pragma unroll
-    for (int e = 0; e < 32; ++e) p[e] = sm.ld(t + T * e);
+        for (int e = 0; e < 32; ++e) p[e].x = sm.ld(t + T * e);
+        sync();
+#pragma unroll
+        for (int r = 0; r < 32; ++r) sm.st(t * 32 + r, p[r].y);
+        sync();
+#pragma unroll
+        for (int e = 0; e < 32; ++e) p[e].y = sm.ld(t + T * e);
+    } else {
+#pragma unroll
+        for (int r = 0; r < 32; ++r) sm.st(t * 32 + r, p[r]);
+        sync();
+#pragma unroll
+        for (int e = 0; e < 32; ++e) p[e] = sm.ld(t + T * e);
+    }
 #pragma unroll
     for (int m = 0; m < P::NB2; ++m) {
         C2 a[P::R2];
@@ -233,10 +271,10 @@ __device__ __forceinline__ void fft_half(C2 (&p)[32], const float2* __restrict__
 // XBE = 32 keeps everything.
 template <int XBE> __device__ __forceinline__ constexpr bool kept(int e) { return e < XBE || e >= 64 - XBE; }
 
-// Forward DIF: v (L1; slots not kept<IN>() are taken as exact zeros) -> p (L2 pairs).
-template <class P, int IN, class SYNC>
-__device__ __forceinline__ void fft_dif(const float2 (&v)[64], C2 (&p)[32], const float2* __restrict__ tab, int t,
-                                        const Xchg& sm, SYNC sync)
+// Radix-2 step of the DIF form: v (L1; slots not kept<IN>() are taken as exact zeros) -> p (pairs (a, b) whose
+// half-length transforms are the even and the odd outputs).
+template <class P, int IN>
+__device__ __forceinline__ void dif_pre(const float2 (&v)[64], C2 (&p)[32], const float2* __restrict__ tab, int t)
 {
     const float2* tn = tab + P::TW2;
 #pragma unroll
@@ -252,15 +290,13 @@ __device__ __forceinline__ void fft_dif(const float2 (&v)[64], C2 (&p)[32], cons
         const float2 b = make_float2(fmaf(d.x, w.x, -d.y * w.y), fmaf(d.x, w.y, d.y * w.x));
         p[e] = { make_float2(a.x, b.x), make_float2(a.y, b.y) };
     }
-    fft_half<P>(p, tab, t, sm, sync);
 }
 
-// Forward DIT: p (L2 pairs) -> v (L1); only slots kept<OUT>() are computed.
-template <class P, int OUT, class SYNC>
-__device__ __forceinline__ void fft_dit(C2 (&p)[32], float2 (&v)[64], const float2* __restrict__ tab, int t,
-                                        const Xchg& sm, SYNC sync)
+// Radix-2 step of the DIT form: p (half-length transforms of the even and odd inputs) -> v (L1); only slots
+// kept<OUT>() are computed.
+template <class P, int OUT>
+__device__ __forceinline__ void dit_post(const C2 (&p)[32], float2 (&v)[64], const float2* __restrict__ tab, int t)
 {
-    fft_half<P>(p, tab, t, sm, sync);
     const float2* tn = tab + P::TW2;
 #pragma unroll
     for (int e = 0; e < 32; ++e) {
@@ -271,6 +307,24 @@ __device__ __forceinline__ void fft_dit(C2 (&p)[32], float2 (&v)[64], const floa
         if (kept<OUT>(e)) v[e] = make_float2(a.x + bw.x, a.y + bw.y);
         if (kept<OUT>(e + 32)) v[e + 32] = make_float2(a.x - bw.x, a.y - bw.y);
     }
+}
+
+// Forward DIF: v (L1) -> p (L2 pairs).
+template <class P, int IN, class SM, class SYNC>
+__device__ __forceinline__ void fft_dif(const float2 (&v)[64], C2 (&p)[32], const float2* __restrict__ tab, int t,
+                                        const SM& sm, SYNC sync)
+{
+    dif_pre<P, IN>(v, p, tab, t);
+    fft_half<P>(p, tab, t, sm, sync);
+}
+
+// Forward DIT: p (L2 pairs) -> v (L1).
+template <class P, int OUT, class SM, class SYNC>
+__device__ __forceinline__ void fft_dit(C2 (&p)[32], float2 (&v)[64], const float2* __restrict__ tab, int t,
+                                        const SM& sm, SYNC sync)
+{
+    fft_half<P>(p, tab, t, sm, sync);
+    dit_post<P, OUT>(p, v, tab, t);
 }
 
 }  // namespace pk

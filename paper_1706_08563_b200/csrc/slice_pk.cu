@@ -34,7 +34,7 @@ struct RowPkCfg {
     static constexpr int T = P::T, LPW = 32 / T;                   // threads per line, lines per warp
     static constexpr int LANDW = XBE < 32 ? 2 * XBE * T : N;       // points of a line that are moved
     static constexpr int LAND_BYTES = LPW * LANDW * 8;
-    static constexpr int X_BYTES = LPW * P::XPAD * 16;
+    static constexpr int X_BYTES = LPW * P::XPAD * 8;               // one 8-byte plane, used in two phases
     static constexpr int PER_WARP = LAND_BYTES + X_BYTES;
     static constexpr int TWB = round_up_c(P::TW_BYTES, 128);
     static constexpr int BY_SMEM = (PIPE_SMEM_MAX - PIPE_HEADER - TWB) / PER_WARP;
@@ -56,7 +56,7 @@ __global__ void __launch_bounds__(RowPkCfg<N, XBE>::THREADS, 1) row_pk_kernel(Ro
     const int ll = lane / T, t = lane % T;
     unsigned char* mine = smem_raw + PIPE_HEADER + C::TWB + (size_t)warp * C::PER_WARP;
     float2* land = reinterpret_cast<float2*>(mine);                            // [LPW][LANDW]
-    float4* xch = reinterpret_cast<float4*>(mine + C::LAND_BYTES);             // [LPW][XPAD]
+    float2* xch = reinterpret_cast<float2*>(mine + C::LAND_BYTES);             // [LPW][XPAD]
 
     pk::fill_tables<P>(tab, g.tw_x, tid, C::THREADS);
     if (MODE != ROW_INIT && lane == 0) { mbar_init(&bars[warp], 1); mbar_fence_init(); }
@@ -87,7 +87,7 @@ __global__ void __launch_bounds__(RowPkCfg<N, XBE>::THREADS, 1) row_pk_kernel(Ro
     };
     if (MODE != ROW_INIT && lane == 0 && gw < n_groups) issue(gw);
 
-    const pk::Xchg sm{ xch + ll * P::XPAD, 1 };
+    const pk::XchgPhase sm{ xch + ll * P::XPAD, 1 };
     auto sync = [] { __syncwarp(); };
     auto in_band = [&](int e) { return XBE < 32 ? pk::kept<XBE>(e) : (t + T * e < xb || t + T * e >= N - xb); };
 
@@ -100,61 +100,69 @@ __global__ void __launch_bounds__(RowPkCfg<N, XBE>::THREADS, 1) row_pk_kernel(Ro
         float2* row = g.a + ((size_t)w * g.ny + y) * N;
         C2 p[32];
 
-        if (MODE == ROW_INIT) {
-            // plane wave exp(+2 pi i (kx x / nx + ky y / ny)) * amplitude at x = 2 j, 2 j + 1
-            const int2 b = g.beams[w];
-            const float2 wy = __ldg(g.tw_y + ((b.y * y) & (g.ny - 1)));
-            const float2 base = make_float2(wy.x * g.scale, -wy.y * g.scale);
+        // Phase 0 builds the pairs the first half-length transform runs on (plane wave, or the landed line after
+        // the radix-2 step of the inverse DIF); phase 1 multiplies by t_s between the inverse and the forward
+        // transform.  ROW_STEP runs both phases through ONE copy of the transform code (instruction cache).
+        constexpr int PH0 = (MODE == ROW_INIT) ? 1 : 0, PH1 = (MODE == ROW_FINAL) ? 1 : 2;
+#pragma unroll 1
+        for (int ph = PH0; ph < PH1; ++ph) {
+            if (ph == 0) {
+                float2 v[64];
+                mbar_wait(&bars[warp], (unsigned)(it & 1));
+                const float2* lbase = land + ll * C::LANDW;
 #pragma unroll
-            for (int e = 0; e < 32; ++e) {
-                const int x0 = 2 * (t + T * e);
-                const float2 w0 = __ldg(g.tw_x + ((b.x * x0) & (N - 1)));
-                const float2 w1 = __ldg(g.tw_x + ((b.x * (x0 + 1)) & (N - 1)));
-                const float2 v0 = cmul_conj(base, w0), v1 = cmul_conj(base, w1);
-                p[e] = { make_float2(v0.x, v1.x), make_float2(v0.y, v1.y) };
+                for (int e = 0; e < 64; ++e) {
+                    const int kx = t + T * e;
+                    int pos;                                    // compact landing: [0, xb) then [N - xb, N)
+                    if (XBE < 32) pos = e < XBE ? kx : kx - (N - 2 * xb);
+                    else pos = kx < xb ? kx : (kx >= N - xb ? kx - (N - 2 * xb) : 0);
+                    if (XBE < 32 && !pk::kept<XBE>(e)) { v[e] = make_float2(0.f, 0.f); continue; }
+                    const float2 q = lbase[pos];
+                    v[e] = in_band(e) ? make_float2(q.y, q.x) : make_float2(0.f, 0.f);   // (im, re): inverse = swapped forward
+                }
+                // the landing buffer is free once every lane has read its points
+                __syncwarp();
+                if (lane == 0 && grp + gstride < n_groups) { fence_proxy_async(); issue(grp + gstride); }
+                pk::dif_pre<P, XBE>(v, p, tab, t);
+            } else {
+                if (MODE == ROW_INIT) {
+                    // plane wave exp(+2 pi i (kx x / nx + ky y / ny)) * amplitude at x = 2 j, 2 j + 1
+                    const int2 b = g.beams[w];
+                    const float2 wy = __ldg(g.tw_y + ((b.y * y) & (g.ny - 1)));
+                    const float2 base = make_float2(wy.x * g.scale, -wy.y * g.scale);
+#pragma unroll
+                    for (int e = 0; e < 32; ++e) {
+                        const int x0 = 2 * (t + T * e);
+                        const float2 w0 = __ldg(g.tw_x + ((b.x * x0) & (N - 1)));
+                        const float2 w1 = __ldg(g.tw_x + ((b.x * (x0 + 1)) & (N - 1)));
+                        const float2 v0 = cmul_conj(base, w0), v1 = cmul_conj(base, w1);
+                        p[e] = { make_float2(v0.x, v1.x), make_float2(v0.y, v1.y) };
+                    }
+                } else {
+#pragma unroll
+                    for (int e = 0; e < 32; ++e) p[e] = pk::cswap(p[e]);       // back from the swapped inverse
+                }
+                // transmission function in pair layout: (re(2j), re(2j+1), im(2j), im(2j+1))
+                const float4* trow = reinterpret_cast<const float4*>(g.t) + (size_t)y * (N / 2);
+#pragma unroll
+                for (int e = 0; e < 32; ++e) {
+                    const float4 q = __ldg(trow + t + T * e);
+                    p[e] = pk::cmul2(p[e], make_float2(q.x, q.y), make_float2(q.z, q.w));
+                }
             }
-        } else {
-            float2 v[64];
-            mbar_wait(&bars[warp], (unsigned)(it & 1));
-            const float2* lbase = land + ll * C::LANDW;
-#pragma unroll
-            for (int e = 0; e < 64; ++e) {
-                const int kx = t + T * e;
-                int pos;                                    // compact landing: [0, xb) then [N - xb, N)
-                if (XBE < 32) pos = e < XBE ? kx : kx - (N - 2 * xb);
-                else pos = kx < xb ? kx : (kx >= N - xb ? kx - (N - 2 * xb) : 0);
-                if (XBE < 32 && !pk::kept<XBE>(e)) { v[e] = make_float2(0.f, 0.f); continue; }
-                const float2 q = lbase[pos];
-                v[e] = in_band(e) ? make_float2(q.y, q.x) : make_float2(0.f, 0.f);   // (im, re): inverse = swapped forward
-            }
-            // the landing buffer is free once every lane has read its points
-            __syncwarp();
-            if (lane == 0 && grp + gstride < n_groups) { fence_proxy_async(); issue(grp + gstride); }
-            pk::fft_dif<P, XBE>(v, p, tab, t, sm, sync);
-#pragma unroll
-            for (int e = 0; e < 32; ++e) p[e] = pk::cswap(p[e]);
-        }
-
-        if (MODE == ROW_INIT || MODE == ROW_STEP) {
-            // transmission function in pair layout: (re(2j), re(2j+1), im(2j), im(2j+1))
-            const float4* trow = reinterpret_cast<const float4*>(g.t) + (size_t)y * (N / 2);
-#pragma unroll
-            for (int e = 0; e < 32; ++e) {
-                const float4 q = __ldg(trow + t + T * e);
-                p[e] = pk::cmul2(p[e], make_float2(q.x, q.y), make_float2(q.z, q.w));
-            }
+            pk::fft_half<P>(p, tab, t, sm, sync);
         }
 
         if (MODE == ROW_FINAL) {
             float4* dst = reinterpret_cast<float4*>(g.out + ((size_t)w * g.ny + y) * N);
             if (active) {
 #pragma unroll
-                for (int e = 0; e < 32; ++e)
-                    dst[t + T * e] = make_float4(p[e].x.x * g.scale, p[e].y.x * g.scale, p[e].x.y * g.scale, p[e].y.y * g.scale);
+                for (int e = 0; e < 32; ++e)       // p holds the swapped inverse: (y, x) are (re, im)
+                    dst[t + T * e] = make_float4(p[e].y.x * g.scale, p[e].x.x * g.scale, p[e].y.y * g.scale, p[e].x.y * g.scale);
             }
         } else {
             float2 v[64];
-            pk::fft_dit<P, XBE>(p, v, tab, t, sm, sync);
+            pk::dit_post<P, XBE>(p, v, tab, t);
             if (active) {
 #pragma unroll
                 for (int e = 0; e < 64; ++e)
@@ -296,7 +304,7 @@ __global__ void __launch_bounds__(ColPkCfg<N>::THREADS, 1) col_pk_kernel(ColArgs
         const int kxi = kx0 + c;                                   // array slot of this thread's column
         const int bi = LOADS ? (int)(k % C::NBUF) : tm;
         unsigned char* buf = bufs + (size_t)bi * C::BUF_BYTES;
-        const pk::Xchg sm{ reinterpret_cast<float4*>(buf) + c, W };
+        const pk::Xchg16 sm{ reinterpret_cast<float4*>(buf) + c, W };
         C2 p[32];
 
         if (MODE == COL_MS_INIT) {
