@@ -46,6 +46,20 @@ def measured_peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
+def measured_traffic(workload: str, kernel: str):
+    """DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of one `ncu --set full` capture of this
+    kernel on this workload, from profiles/r01_traffic.csv (the .md beside it names the commands); None if absent."""
+    path = os.path.join(ROOT, "profiles", "r01_traffic.csv")
+    if not os.path.exists(path):
+        return None
+    with open(path) as fh:
+        for line in fh:
+            f = [x.strip() for x in line.split(",")]
+            if len(f) >= 3 and f[0] == workload and f[1] == kernel:
+                return float(f[2])
+    return None
+
+
 # ------------------------------------------------------------------------------------------------ clocks
 class ClockSampler(threading.Thread):
     """Samples SM clock and throttle reasons through NVML while the timed region runs."""
@@ -222,6 +236,12 @@ def main():
     ws_bytes = max(prism.workspace_bytes(p, prism.WS_POTENTIAL, len(w.z)), prism.workspace_bytes(p, prism.WS_SMATRIX),
                    prism.workspace_bytes(p, prism.WS_OUTPUT))
     ws = torch.empty(ws_bytes, dtype=torch.uint8, device=dev)
+    # comparison path: plain multislice on a coarse sub-grid of the probe positions
+    ms_n = max(1, min(8, w.probes_x, w.probes_y))
+    w_ms = w.with_(probes_x=ms_n, probes_y=ms_n, probe_step=(w.cell[0] / ms_n, w.cell[1] / ms_n))
+    p_ms = prism.params_from_workload(w_ms)
+    out_ms = torch.empty((ms_n, ms_n, n_bins), dtype=torch.float32, device=dev)
+    ws_ms = torch.empty(prism.workspace_bytes(p_ms, prism.WS_MULTISLICE), dtype=torch.uint8, device=dev)
     # frozen-phonon configurations of this rank (host inputs, prepared outside the timed region)
     my_phonons = [ph for ph in range(max(w.n_phonons, world)) if ph % world == rank]
     atoms = {ph: np.ascontiguousarray(w.atoms_for_phonon(ph)) for ph in my_phonons}
@@ -290,6 +310,16 @@ def main():
         t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         e2e_s = float(t.item())
+    # ---- comparison path: multislice probes/s on ms_n x ms_n probes through the same slice-step kernels ----
+    prism.multislice_output(p_ms, v, out_ms, ws_ms)                  # warm-up
+    barrier()
+    m0, m1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    m0.record()
+    prism.multislice_output(p_ms, v, out_ms, ws_ms)
+    m1.record()
+    barrier()
+    ms_probes_per_s = world * ms_n * ms_n / (m0.elapsed_time(m1) * 1e-3)
+    del ws_ms
     cells = w.n_slices * (w.nx // 16) * (w.ny // 16)
     v_bytes = 4 * npix * w.n_slices if w.potential_on_host else 0
     h2d = 24 * len(w.z) + 4 * (cells + 1) + lut_v.size * 4 + v_bytes + 8 * (2 * w.nx + 2 * w.ny) \
@@ -322,7 +352,7 @@ def main():
     if top in per_launch_bytes:
         ach = kernels[top]["algorithmic_GBps"]
         roofline = {"kernel": top, "bound": "hbm", "achieved": ach, "peak": hbm_peak, "unit": "GB/s",
-                    "frac": ach / hbm_peak, "traffic": None, "peak_source": peak_src,
+                    "frac": ach / hbm_peak, "traffic": measured_traffic(w.name, top), "peak_source": peak_src,
                     "bytes_per_launch": per_launch_bytes[top]}
     else:
         ach = kernels[top].get("algorithmic_TFLOPs", 0.0)
@@ -348,6 +378,10 @@ def main():
         "beam_slices_per_s": world * n_beams * w.n_slices / (stage_ms[1] * 1e-3),
         "stage2_probes_per_s": world * n_probes / (stage_ms[2] * 1e-3),
         "stage_ms": {"potential": stage_ms[0], "smatrix": stage_ms[1], "output": stage_ms[2]},
+        "multislice": {"probes_per_s": ms_probes_per_s, "probes": ms_n * ms_n,
+                       "note": "comparison path (row M1): same potential and slice-step kernels, one probe per wave; "
+                               "PRISM / multislice speed-up = stage2_probes_per_s / probes_per_s once the S-matrix is built",
+                       "prism_over_multislice": (world * n_probes / (ms_per_step * 1e-3)) / ms_probes_per_s},
         "roofline": roofline, "kernels": kernels,
     }
     if world == 1 and not args.no_cpu_baseline:

@@ -31,72 +31,76 @@
 
 namespace prism {
 
+#ifndef ROW_MAX_TEAMS
+#define ROW_MAX_TEAMS 16
+#endif
+
 // =============================================================================
 // Row pass
 // =============================================================================
-template <class P>
+// A team is one warp holding LPT = 32 / T lines.  Per team: one landing buffer the TMA engine fills with the
+// in-band points of the next line group (compact: [0, xb) then [N - xb, N)) and one exchange space.  The
+// landing buffer is refilled as soon as the group is in registers, so the copy of group i + 1 overlaps the
+// whole computation of group i.  XBE > 0: the band is xband = XBE * T columns, known at compile time (then
+// "in band" depends on the register index e only and out-of-band elements cost no instruction); XBE = 0: any
+// xband, tested per element.
+template <class P, int XBE>
 struct RowCfg {
     static constexpr int T = P::T;
-    static constexpr int TEAM = T < 32 ? 32 : T;                 // threads of one team
-    static constexpr int LPT = TEAM / T;                         // lines per team
+    static_assert(T <= 32, "one warp per line group");
+    static constexpr int LPT = 32 / T;                           // lines per team
     static constexpr int LINE = P::N + 2 * (P::N / P::R1);       // padded exchange space of one line (float2)
-    static constexpr int SLOT = LPT * LINE;
+    static constexpr int LANDW = XBE > 0 ? 2 * XBE * T : P::N;   // points of a line that are moved
+    static constexpr int PER_TEAM = LPT * (LINE + LANDW) * 8;
     static constexpr int TWB = round_up_c(SmemTwiddles<P>::COUNT * 8, 128);
-    static constexpr int TEAMS_BY_SMEM = (PIPE_SMEM_MAX - PIPE_HEADER - TWB) / (2 * SLOT * 8);
-    static constexpr int TEAMS = TEAMS_BY_SMEM < 384 / TEAM ? TEAMS_BY_SMEM : 384 / TEAM;
-    static constexpr int THREADS = TEAMS * TEAM;
-    static constexpr size_t SMEM = PIPE_HEADER + TWB + (size_t)TEAMS * 2 * SLOT * 8;
+    static constexpr int TEAMS_BY_SMEM = (PIPE_SMEM_MAX - PIPE_HEADER - TWB) / PER_TEAM;
+    static constexpr int TEAMS = TEAMS_BY_SMEM < ROW_MAX_TEAMS ? TEAMS_BY_SMEM : ROW_MAX_TEAMS;
+    static constexpr int THREADS = TEAMS * 32;
+    static constexpr size_t SMEM = PIPE_HEADER + TWB + (size_t)TEAMS * PER_TEAM;
 };
 
-// exchange space of one line inside its slot: element idx at base[idx + 2 (idx / R1)].  Two pad words per
-// group of R1 keep pairs (even idx, idx + 1) 16-byte aligned, so the radix-R1 outputs of a thread go out as
-// 16-byte stores, and a quarter warp of such stores (stride R1 + 2 words) covers all banks once.
-template <class P, int TEAM>
+// exchange space of one line: element idx at base[idx + 2 (idx / R1)].  Two pad words per group of R1 keep
+// pairs (even idx, idx + 1) 16-byte aligned, so the radix-R1 outputs of a thread go out as 16-byte stores, and
+// a quarter warp of such stores (stride R1 + 2 words) covers all banks once.
+template <class P>
 struct RowSm {
     float2* base;
-    int bar_id;
     __device__ __forceinline__ static int phys(int idx) { return idx + 2 * (idx / P::R1); }
     __device__ __forceinline__ void  st(int idx, float2 v) const { base[phys(idx)] = v; }
     __device__ __forceinline__ void  st2(int idx, float2 v0, float2 v1) const
     { *reinterpret_cast<float4*>(base + phys(idx)) = make_float4(v0.x, v0.y, v1.x, v1.y); }
     __device__ __forceinline__ float2 ld(int idx) const { return base[phys(idx)]; }
-    __device__ __forceinline__ void sync() const { if (TEAM <= 32) __syncwarp(); else named_barrier(bar_id, TEAM); }
+    __device__ __forceinline__ void sync() const { __syncwarp(); }
 };
 
-// XBE > 0: the band is xband = XBE * T columns, known at compile time (then "in band" depends on the register
-// index e only and out-of-band elements cost no instruction); XBE = 0: any xband, tested per element.
 template <class P, int MODE, int XBE>
-__global__ void __launch_bounds__(RowCfg<P>::THREADS, 1) row_pipe_kernel(RowArgs g)
+__global__ void __launch_bounds__(RowCfg<P, XBE>::THREADS, 1) row_pipe_kernel(RowArgs g)
 {
-    using C = RowCfg<P>;
+    using C = RowCfg<P, XBE>;
     constexpr int E = P::E, T = P::T, N = P::N;
     auto in_band = [&](int e, int kx, int xb) { return XBE > 0 ? (e < XBE || e >= E - XBE) : (kx < xb || kx >= N - xb); };
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw);                    // [TEAMS][2]
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw);                    // [TEAMS]
     float2* twtab = reinterpret_cast<float2*>(smem_raw + PIPE_HEADER);
-    float2* slots = reinterpret_cast<float2*>(smem_raw + PIPE_HEADER + C::TWB);
-    const int tid = threadIdx.x, team = tid / C::TEAM, tt = tid % C::TEAM;
+    const int tid = threadIdx.x, team = tid >> 5, tt = tid & 31;
     const int ll = tt / T, t = tt % T;
+    float2* land = reinterpret_cast<float2*>(smem_raw + PIPE_HEADER + C::TWB + (size_t)team * C::PER_TEAM);   // [LPT][LANDW]
+    float2* xch = land + C::LPT * C::LANDW;                                                                    // [LPT][LINE]
 
     SmemTwiddles<P>::fill(twtab, g.tw_x, tid, C::THREADS);
-    if (MODE != ROW_INIT && tt == 0) {
-        mbar_init(&bars[team * 2], 1);
-        mbar_init(&bars[team * 2 + 1], 1);
-        mbar_fence_init();
-    }
+    if (MODE != ROW_INIT && tt == 0) { mbar_init(&bars[team], 1); mbar_fence_init(); }
     __syncthreads();
     SmemTwiddles<P> tw;
     tw.bind(twtab, t);
-    float2* slot0 = slots + (size_t)team * 2 * C::SLOT;
 
     const long long n_lines = (long long)g.n_waves * g.ny;
     const long long n_groups = (n_lines + C::LPT - 1) / C::LPT;
     const long long gteam = (long long)blockIdx.x * C::TEAMS + team, gstride = (long long)gridDim.x * C::TEAMS;
     const int xb = XBE > 0 ? XBE * T : g.xband;              // in-band columns: [0, xb) and [N - xb, N)
 
-    // one thread of the team: start the bulk copies of line group `grp` into slot `s`
-    auto issue = [&](long long grp, int s) {
-        uint64_t* bar = &bars[team * 2 + s];
+    // one thread of the team: start the bulk copies of line group `grp` into the landing buffer
+    auto issue = [&](long long grp) {
+        uint64_t* bar = &bars[team];
         int n_act = 0;
 #pragma unroll
         for (int l = 0; l < C::LPT; ++l) n_act += (grp * C::LPT + l < n_lines);
@@ -107,27 +111,22 @@ __global__ void __launch_bounds__(RowCfg<P>::THREADS, 1) row_pipe_kernel(RowArgs
             if (line < n_lines) {
                 const int y = (int)(line / g.n_waves), w = (int)(line % g.n_waves);
                 const float2* row = g.a + ((size_t)w * g.ny + y) * N;
-                float2* dst = slot0 + s * C::SLOT + l * C::LINE;
+                float2* dst = land + l * C::LANDW;
                 bulk_g2s(dst, row, (unsigned)(xb * sizeof(float2)), bar);
-                bulk_g2s(dst + (N - xb), row + (N - xb), (unsigned)(xb * sizeof(float2)), bar);
+                bulk_g2s(dst + xb, row + (N - xb), (unsigned)(xb * sizeof(float2)), bar);
             }
         }
     };
-    if (MODE != ROW_INIT && tt == 0) {
-        if (gteam < n_groups) issue(gteam, 0);
-        if (gteam + gstride < n_groups) issue(gteam + gstride, 1);
-    }
+    if (MODE != ROW_INIT && tt == 0 && gteam < n_groups) issue(gteam);
 
+    const RowSm<P> sm{ xch + ll * C::LINE };
     int it = 0;
     for (long long grp = gteam; grp < n_groups; grp += gstride, ++it) {
-        const int s = it & 1;
         long long line = grp * C::LPT + ll;
         const bool active = line < n_lines;
         if (!active) line = n_lines - 1;                 // keep every thread in the barriers
         const int y = (int)(line / g.n_waves), w = (int)(line % g.n_waves);
         float2* row = g.a + ((size_t)w * g.ny + y) * N;
-        float2* lbase = slot0 + s * C::SLOT + ll * C::LINE;
-        const RowSm<P, C::TEAM> sm{ lbase, 1 + team };
         float2 v[E];
 
         if (MODE == ROW_INIT) {
@@ -141,12 +140,21 @@ __global__ void __launch_bounds__(RowCfg<P>::THREADS, 1) row_pipe_kernel(RowArgs
                 v[e] = cmul_conj(base, wx);
             }
         } else {
-            mbar_wait(&bars[team * 2 + s], (unsigned)((it >> 1) & 1));
+            mbar_wait(&bars[team], (unsigned)(it & 1));
+            const float2* lbase = land + ll * C::LANDW;
 #pragma unroll
             for (int e = 0; e < E; ++e) {
                 const int kx = t + T * e;
-                v[e] = in_band(e, kx, xb) ? lbase[kx] : make_float2(0.f, 0.f);   // out of band: exact zeros
+                int pos;                                    // compact landing: [0, xb) then [N - xb, N)
+                if (XBE > 0) pos = e < XBE ? kx : kx - (N - 2 * xb);
+                else pos = kx < xb ? kx : (kx >= N - xb ? kx - (N - 2 * xb) : 0);
+                if (XBE > 0 && !in_band(e, kx, xb)) { v[e] = make_float2(0.f, 0.f); continue; }
+                const float2 q = lbase[pos];
+                v[e] = in_band(e, kx, xb) ? q : make_float2(0.f, 0.f);            // out of band: exact zeros
             }
+            // the landing buffer is free once every lane has read its points
+            __syncwarp();
+            if (tt == 0 && grp + gstride < n_groups) { fence_proxy_async(); issue(grp + gstride); }
         }
 
         if (MODE == ROW_STEP || MODE == ROW_FINAL) fft_inverse<P>(v, tw, t, sm);
@@ -157,15 +165,6 @@ __global__ void __launch_bounds__(RowCfg<P>::THREADS, 1) row_pipe_kernel(RowArgs
             for (int e = 0; e < E; ++e) v[e] = cmul(v[e], __ldg(trow + t + T * e));
         }
         if (MODE != ROW_FINAL) fft_forward<P>(v, tw, t, sm);
-
-        if (MODE != ROW_INIT) {
-            // the slot is free once every thread of the team is past its last exchange read
-            sm.sync();
-            if (tt == 0) {
-                const long long nxt = grp + 2 * gstride;
-                if (nxt < n_groups) { fence_proxy_async(); issue(nxt, s); }
-            }
-        }
 
         if (MODE == ROW_FINAL) {
             float2* dst = g.out + ((size_t)w * g.ny + y) * N;
@@ -186,7 +185,7 @@ __global__ void __launch_bounds__(RowCfg<P>::THREADS, 1) row_pipe_kernel(RowArgs
 template <class P, int MODE, int XBE>
 static cudaError_t launch_row_pipe_x(const RowArgs& g, cudaStream_t stream)
 {
-    using C = RowCfg<P>;
+    using C = RowCfg<P, XBE>;
     auto kern = row_pipe_kernel<P, MODE, XBE>;
     static bool set = false;
     if (!set) {
@@ -233,7 +232,6 @@ cudaError_t launch_row_pipe(RowMode mode, const RowArgs& g, cudaStream_t stream)
         case 256:  return launch_row_pipe_n<256>(mode, g, stream);
         case 512:  return launch_row_pipe_n<512>(mode, g, stream);
         case 1024: return launch_row_pipe_n<1024>(mode, g, stream);
-        case 2048: return launch_row_pipe_n<2048>(mode, g, stream);
     }
     return cudaErrorInvalidValue;
 }

@@ -1,0 +1,159 @@
+"""Parity at BASELINE.json's full sizes, in the launch configuration bench.py times (whole beam set resident,
+library-default batches, streamed potential for P16), on sampled outputs the oracle can compute one by one
+(SURVEY.md 8(d) "parity by decomposition"):
+
+  * the whole potential stack against the oracle's;
+  * sampled S-matrix layers against oracle layers (each is one plane wave through every slice);
+  * sampled probes of stage 2 against the oracle's stage 2 applied to the GPU S-matrix (fp64 copy);
+  * sampled multislice probes end to end.
+
+Tolerances: output rings 1e-4 relative L2 (1e-3 at 2048^2 with >= 400 slices), BASELINE.json north_star;
+S-matrix layers 3e-7 sqrt(S) x 20; stage 2 in isolation 2e-5.
+
+The 400-slice 2048^2 oracle costs ~8 core-minutes per wave, so the default suite runs config 5 on its first
+40 slices (same grid, beams, streaming ring, kernels) and the full 400-slice case runs with
+PRISM_FULL_P16=1 (its last recorded result is in DESIGN.md section 5)."""
+import math
+import os
+
+import numpy as np
+import pytest
+
+import oracle as O
+from helpers import oracle_params, oracle_potential, rel_l2
+from paper_1706_08563_b200 import workloads as W
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+TOL_OUT = 1e-4
+TOL_V = 1e-6
+TOL_STAGE2 = 2e-5
+
+
+def tol_layer(n_slices):
+    return 20.0 * 3e-7 * math.sqrt(n_slices)
+
+
+@pytest.fixture(scope="module")
+def G():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import gpu_helpers
+    return gpu_helpers
+
+
+def spread(n, k):
+    return np.unique(np.linspace(0, n - 1, k).astype(int))
+
+
+def check_prism(G, w, n_layers, n_probes, beam_filter=None, tol_out=TOL_OUT):
+    """Potential, sampled layers, stage 2 on sampled probes.  beam_filter(beams) -> mask selects the layers
+    stage 2 is run on when the fp64 copy of the whole S-matrix would not fit in host memory."""
+    p = oracle_params(w)
+    on_host = bool(w.potential_on_host)
+    v = G.gpu_potential(w, on_host=on_host)
+    v_ref = oracle_potential(w)
+    v_gpu = v.cpu().numpy() if not on_host else v.numpy()
+    assert rel_l2(v_gpu.astype(np.float64), v_ref) < TOL_V
+    del v_gpu
+    s, beams = G.gpu_smatrix(w, v)
+    ref_beams = O.beams(p)
+    assert set(map(tuple, beams.tolist())) == set(map(tuple, ref_beams.tolist()))
+    pick = spread(len(beams), n_layers)
+    layers = O.smatrix(p, v_ref, beams[pick])
+    errs = [rel_l2(s[b].cpu().numpy().astype(np.complex128), layers[i]) for i, b in enumerate(pick)]
+    assert max(errs) < tol_layer(w.n_slices), errs
+    del layers
+    # stage 2 in isolation on the layers the host can hold in fp64
+    if beam_filter is None:
+        sel = np.arange(len(beams))
+        s_sel = s
+    else:
+        sel = np.nonzero(beam_filter(beams))[0]
+        s_sel = s[torch.as_tensor(sel, device=s.device)].contiguous()
+    out = G.gpu_prism_output(w, s_sel, np.ascontiguousarray(beams[sel]))
+    xy = w.probe_xy()
+    rows = spread(len(xy), n_probes)
+    s64 = s_sel.cpu().numpy().astype(np.complex128)
+    ref = O.prism_probes(p, s64, np.ascontiguousarray(beams[sel]), xy[rows])
+    assert rel_l2(out[rows], ref) < TOL_STAGE2
+    d = G.dark_field(w, p)
+    assert ref[:, d:].sum() > 0
+    assert rel_l2(out[rows][:, d:], ref[:, d:]) < 5 * tol_out
+    # every probe of the grid: the rings hold about the incident current (PRISM's cropped window is not exactly
+    # norm-conserving for f > 1, so this is a sanity band, not an identity)
+    tot = out.sum(axis=1)
+    assert np.all(tot > 0.5) and np.all(tot < 1.05)
+    return v, v_ref, errs
+
+
+def check_multislice(G, w, v, v_ref, n_probes, tol_out=TOL_OUT):
+    p = oracle_params(w)
+    out = G.gpu_multislice(w, v)
+    xy = w.probe_xy()
+    rows = spread(len(xy), n_probes)
+    ref = O.multislice_probes(p, v_ref, xy[rows])
+    e = rel_l2(out[rows], ref)
+    assert e < tol_out, e
+    d = G.dark_field(w, p)
+    assert rel_l2(out[rows][:, d:], ref[:, d:]) < 5 * tol_out
+    tot = out.sum(axis=1)
+    assert np.all(tot > 0.0) and np.all(tot < 1.0 + 1e-4)
+    return e
+
+
+def test_ms2_full(G):
+    """BASELINE.json configs[1]: 256^2, 50 slices, 32 x 32 probes, batches of 64."""
+    w = W.ms2()
+    assert w.batch == 64
+    v = G.gpu_potential(w)
+    v_ref = oracle_potential(w)
+    assert rel_l2(v.cpu().numpy().astype(np.float64), v_ref) < TOL_V
+    check_multislice(G, w, v, v_ref, 48)
+
+
+def test_p4_full(G):
+    """BASELINE.json configs[2]: 512^2, 100 slices, f = 4, 529 beams, 128 x 128 probes."""
+    check_prism(G, W.p4(), n_layers=4, n_probes=12)
+
+
+def test_p8_full(G):
+    """BASELINE.json configs[3]: 1024^2, 50 slices, f = 8, 509 beams, 256 x 256 probes, defocus 50 A."""
+    check_prism(G, W.p8(), n_layers=4, n_probes=12)
+
+
+def p16_cases(n_slices):
+    """Config 5 on its first n_slices slices: atoms above the truncated stack are dropped (not clamped into the
+    last slice), everything else -- grid, beams, streamed potential, probe lattices -- is config 5."""
+    w = W.p16()
+    if n_slices < w.n_slices:
+        keep = w.atoms[:, 2] < n_slices * w.dz - 1.0
+        w = w.with_(n_slices=n_slices, atoms=w.atoms[keep], z=w.z[keep],
+                    cell=(w.cell[0], w.cell[1], n_slices * w.dz))
+    wm = w.with_(name="P16-MS", probes_x=64, probes_y=64, probe_step=(3.2, 3.2))
+    return w, wm
+
+
+def run_p16(G, n_slices, n_layers, n_ms_probes, tol_out):
+    w, wm = p16_cases(n_slices)
+    assert w.potential_on_host == 1 and w.nx == 2048 and w.f == 16
+    # stage 2 on the three central rows of the beam lattice (|ky / f| <= 1): 39 beam columns fold onto the
+    # 32 residues of the probe lattice, so the folded path of the lattice DFT is exercised (117 of 1201 layers)
+    v, v_ref, errs = check_prism(G, w, n_layers=n_layers, n_probes=6,
+                                 beam_filter=lambda b: np.abs(b[:, 1]) <= w.f, tol_out=tol_out)
+    torch.cuda.empty_cache()
+    e = check_multislice(G, wm, v, v_ref, n_ms_probes, tol_out=tol_out)
+    print(f"P16 x {n_slices} slices: S-matrix layer errors {errs}, multislice rings {e:.3e}")
+
+
+def test_p16_first_40_slices(G):
+    """BASELINE.json configs[4] (2048^2, f = 16, 1201 beams, 512 x 512 probes, potential streamed from pinned
+    host memory; multislice on 64 x 64 probes), first 40 of the 400 slices."""
+    run_p16(G, 40, n_layers=2, n_ms_probes=2, tol_out=TOL_OUT)
+
+
+@pytest.mark.skipif(os.environ.get("PRISM_FULL_P16") != "1", reason="~10 min of oracle time: set PRISM_FULL_P16=1")
+def test_p16_full_400_slices(G):
+    """All 400 slices: tolerance 1e-3 on the rings (BASELINE.json north_star)."""
+    run_p16(G, 400, n_layers=2, n_ms_probes=2, tol_out=1e-3)
