@@ -204,7 +204,7 @@ def main():
         return run_reference(args)
 
     import torch
-    from paper_1706_08563_b200 import prism, workloads
+    from paper_1706_08563_b200 import prism, sharding, workloads
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -243,7 +243,7 @@ def main():
     out_ms = torch.empty((ms_n, ms_n, n_bins), dtype=torch.float32, device=dev)
     ws_ms = torch.empty(prism.workspace_bytes(p_ms, prism.WS_MULTISLICE), dtype=torch.uint8, device=dev)
     # frozen-phonon configurations of this rank (host inputs, prepared outside the timed region)
-    my_phonons = [ph for ph in range(max(w.n_phonons, world)) if ph % world == rank]
+    my_phonons = sharding.phonons_for_rank(w.n_phonons, world, rank)
     atoms = {ph: np.ascontiguousarray(w.atoms_for_phonon(ph)) for ph in my_phonons}
     beams_holder = {}
 
@@ -281,8 +281,7 @@ def main():
         prism.compute_output(p, s, beams, out_dev, ws)
         stage_ev[k][3].record()
         acc += out_dev
-    if dist is not None:
-        dist.all_reduce(acc)                                      # frozen-phonon average
+    sharding.phonon_average(acc, args.steps, dist)                # frozen-phonon average
     e1.record()
     barrier()
     ms_total = e0.elapsed_time(e1)

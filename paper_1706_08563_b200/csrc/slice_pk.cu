@@ -24,6 +24,10 @@ namespace prism {
 
 using pk::C2;
 
+#ifndef PK_ROW_MAX_WARPS
+#define PK_ROW_MAX_WARPS 8
+#endif
+
 // =============================================================================
 // Row pass
 // =============================================================================
@@ -38,7 +42,7 @@ struct RowPkCfg {
     static constexpr int PER_WARP = LAND_BYTES + X_BYTES;
     static constexpr int TWB = round_up_c(P::TW_BYTES, 128);
     static constexpr int BY_SMEM = (PIPE_SMEM_MAX - PIPE_HEADER - TWB) / PER_WARP;
-    static constexpr int WARPS = BY_SMEM < 8 ? BY_SMEM : 8;
+    static constexpr int WARPS = BY_SMEM < PK_ROW_MAX_WARPS ? BY_SMEM : PK_ROW_MAX_WARPS;
     static constexpr int THREADS = WARPS * 32;
     static constexpr size_t SMEM = PIPE_HEADER + TWB + (size_t)WARPS * PER_WARP;
 };
