@@ -29,19 +29,25 @@
 
 namespace prism {
 
+#ifndef COL_TILE_PTS
+#define COL_TILE_PTS 8192
+#endif
+
 // =============================================================================
 // Column pass
 // =============================================================================
 template <class P>
 struct ColCfg {
-    static constexpr int TILE_PTS = 8192;
+    static constexpr int TILE_PTS = COL_TILE_PTS;
     static constexpr int W = TILE_PTS / P::N;                    // columns per tile: 32, 16, 8, 4
     static constexpr int TEAM = TILE_PTS / P::E;                 // 256 threads per team
     static constexpr int LPW = 32 / W;                           // threads of one column inside a warp
     static constexpr int ROWS = P::N + P::N / P::R1;             // padded rows
     static constexpr int BUF = ROWS * W;                         // float2 per buffer
-    static constexpr int NBUF = 3;
-    static constexpr int THREADS = 2 * TEAM;
+    static constexpr int NT = 512 / TEAM;                        // teams per CTA
+    static constexpr int THREADS = NT * TEAM;
+    static constexpr int NBUF_FIT = (PIPE_SMEM_MAX - PIPE_HEADER - round_up_c(SmemTwiddles<P>::COUNT * 8, 128)) / (BUF * 8);
+    static constexpr int NBUF = NBUF_FIT < NT + NT / 2 ? NBUF_FIT : NT + NT / 2;   // 3 buffers for 2 teams, 6 for 4
     static constexpr int TWB = round_up_c(SmemTwiddles<P>::COUNT * 8, 128);
     static constexpr size_t SMEM = PIPE_HEADER + TWB + (size_t)NBUF * BUF * 8;
     static_assert(TEAM / 32 * LPW == P::T, "team shape");
@@ -112,11 +118,12 @@ __global__ void __launch_bounds__(ColCfg<P>::THREADS, 1) col_pipe_kernel(ColArgs
         cp_async_arrive(&full[k % C::NBUF]);
     };
     if (LOADS) {
-        if (tm == 0) { if (n_local > 0) load(0); if (n_local > 2) load(2); }
-        else         { if (n_local > 1) load(1); }
+#pragma unroll
+        for (int i = 0; i < C::NBUF; ++i)
+            if (i % C::NT == tm && i < n_local) load(i);
     }
 
-    for (long long k = tm; k < n_local; k += 2) {
+    for (long long k = tm; k < n_local; k += C::NT) {
         int w, kx0;
         locate(k, w, kx0);
         const int kxi = kx0 + c;                                   // array slot of this thread's column
@@ -191,7 +198,7 @@ static cudaError_t launch_col_pipe_s(const ColArgs& g, cudaStream_t stream)
     if (g.xband % C::W || g.nx % C::W) return cudaErrorInvalidValue;
     const long long n_items = (long long)g.n_waves * (2 * g.xband / C::W);
     if (n_items == 0) return cudaSuccess;
-    long long grid = (n_items + 1) / 2;                             // at least one tile per team
+    long long grid = (n_items + C::NT - 1) / C::NT;                 // at least one tile per team
     if (grid > num_sms()) grid = num_sms();
     kern<<<(unsigned)grid, C::THREADS, C::SMEM, stream>>>(g);
     return cudaGetLastError();
@@ -226,7 +233,6 @@ cudaError_t launch_col_pipe(ColMode mode, const ColArgs& g, cudaStream_t stream)
         case 256:  return launch_col_pipe_n<256>(mode, g, stream);
         case 512:  return launch_col_pipe_n<512>(mode, g, stream);
         case 1024: return launch_col_pipe_n<1024>(mode, g, stream);
-        case 2048: return launch_col_pipe_n<2048>(mode, g, stream);
     }
     return cudaErrorInvalidValue;
 }
