@@ -40,12 +40,20 @@ static const char* const kClassNames[K_NUM_CLASSES] = {
 struct TimedLaunch { int cls; cudaEvent_t e0, e1; };
 static bool g_timing = false;
 static std::vector<TimedLaunch> g_timed;
+static std::vector<cudaEvent_t> g_event_pool;      // events are reused: creating them costs more than recording
+static cudaEvent_t take_event()
+{
+    cudaEvent_t e = nullptr;
+    if (!g_event_pool.empty()) { e = g_event_pool.back(); g_event_pool.pop_back(); }
+    else cudaEventCreate(&e);
+    return e;
+}
 
 #define LAUNCH(cls, call, stream)                                                      \
     do {                                                                               \
         cudaEvent_t e0__ = nullptr, e1__ = nullptr;                                    \
         if (g_timing) {                                                                \
-            cudaEventCreate(&e0__); cudaEventCreate(&e1__);                            \
+            e0__ = take_event(); e1__ = take_event();                                  \
             cudaEventRecord(e0__, (stream));                                           \
         }                                                                              \
         cudaError_t e__ = (call);                                                      \
@@ -263,7 +271,10 @@ struct SliceFeeder {
     int n_slices = 0;
     double sigma = 0;
     bool pairs = false;                 // transmission function in pair layout (packed row pass)
-    float2* tbuf = nullptr;
+    float2* tbuf = nullptr;             // t_s of the current slice; or of every slice when t_slices == n_slices
+    int t_slices = 1;                   // slices of t kept (small stacks keep all of them across wave batches)
+    int t_done = 0;                     // slices [0, t_done) of a kept stack are already computed
+    float2* current = nullptr;          // t_s the next passes read
     float* ring[RING] = {nullptr, nullptr, nullptr};
     cudaStream_t main_stream = nullptr, copy_stream = nullptr;
     cudaEvent_t filled[RING] = {}, consumed[RING] = {};
@@ -310,7 +321,14 @@ struct SliceFeeder {
             CU(cudaStreamWaitEvent(main_stream, filled[r], 0));
             src = ring[r];
         }
-        LAUNCH(K_TRANSMISSION, launch_transmission(src, tbuf, sigma, npix, pairs, main_stream), main_stream);
+        if (t_slices > 1) {
+            current = tbuf + (size_t)s * npix;
+            if (s < t_done) return PRISM_OK;        // computed by an earlier wave batch
+            t_done = s + 1;
+        } else {
+            current = tbuf;
+        }
+        LAUNCH(K_TRANSMISSION, launch_transmission(src, current, sigma, npix, pairs, main_stream), main_stream);
         if (on_host) CU(cudaEventRecord(consumed[s % RING], main_stream));
         return PRISM_OK;
     }
@@ -360,7 +378,10 @@ static int fill_slice_tables(const prism_params* p, const SliceTables& t, cudaSt
 static void carve_feeder(Arena& a, const prism_params* p, SliceFeeder& f)
 {
     const size_t npix = (size_t)p->nx * p->ny;
-    f.tbuf = a.take<float2>(npix);
+    // a resident potential whose transmission functions fit in 256 MiB keeps all of them, so that later wave
+    // batches (multislice probes) do not recompute them
+    f.t_slices = (!p->potential_on_host && (size_t)p->n_slices * npix * sizeof(float2) <= ((size_t)256 << 20)) ? p->n_slices : 1;
+    f.tbuf = a.take<float2>(npix * f.t_slices);
     if (p->potential_on_host)
         for (int r = 0; r < SliceFeeder::RING; ++r) f.ring[r] = a.take<float>(npix);
 }
@@ -539,8 +560,8 @@ int prism_timing_read(double* ms_by_class, int64_t* launches_by_class)
         CU(cudaEventElapsedTime(&ms, t.e0, t.e1));
         ms_by_class[t.cls] += ms;
         ++launches_by_class[t.cls];
-        cudaEventDestroy(t.e0);
-        cudaEventDestroy(t.e1);
+        g_event_pool.push_back(t.e0);
+        g_event_pool.push_back(t.e1);
     }
     g_timed.clear();
     return PRISM_OK;
@@ -758,6 +779,7 @@ int prism_compute_smatrix(const prism_params* p, const float* v, int32_t* beams_
             for (int sl = 0; sl < p->n_slices; ++sl) {
                 int r = feed.get(sl);
                 if (r) return r;
+                ra.t = feed.current;
                 if (sl == 0) {
                     ra.scale = (float)p->nx;                 // keeps A' = nx * FFT_x(t psi), see DESIGN.md
                     LAUNCH(K_ROW_INIT, launch_row_pass(ROW_INIT, ra, st), st);
@@ -988,6 +1010,7 @@ int multislice_compute_output(const prism_params* p, const float* v, float* out,
             for (int sl = 0; sl < p->n_slices; ++sl) {
                 int r = feed.get(sl);
                 if (r) return r;
+                ra.t = feed.current;
                 LAUNCH(K_ROW_STEP, launch_row_pass(ROW_STEP, ra, st), st);
                 if (sl == p->n_slices - 1) LAUNCH(K_COL_MS_FINAL, launch_col_pass(COL_MS_FINAL, ca, st), st);
                 else LAUNCH(K_COL_STEP, launch_col_pass(COL_STEP, ca, st), st);
