@@ -375,12 +375,12 @@ static int fill_slice_tables(const prism_params* p, const SliceTables& t, cudaSt
     CU(upload(t.ky_lim, lim, st));
     return PRISM_OK;
 }
-static void carve_feeder(Arena& a, const prism_params* p, SliceFeeder& f)
+static void carve_feeder(Arena& a, const prism_params* p, SliceFeeder& f, bool many_batches)
 {
     const size_t npix = (size_t)p->nx * p->ny;
     // a resident potential whose transmission functions fit in 256 MiB keeps all of them, so that later wave
     // batches (multislice probes) do not recompute them
-    f.t_slices = (!p->potential_on_host && (size_t)p->n_slices * npix * sizeof(float2) <= ((size_t)256 << 20)) ? p->n_slices : 1;
+    f.t_slices = (many_batches && !p->potential_on_host && (size_t)p->n_slices * npix * sizeof(float2) <= ((size_t)256 << 20)) ? p->n_slices : 1;
     f.tbuf = a.take<float2>(npix * f.t_slices);
     if (p->potential_on_host)
         for (int r = 0; r < SliceFeeder::RING; ++r) f.ring[r] = a.take<float>(npix);
@@ -391,7 +391,7 @@ struct SmatrixLayout { SliceTables tab; SliceFeeder feed; int2* beams; };
 static void layout_smatrix(Arena& a, const prism_params* p, int n_beams, SmatrixLayout& L)
 {
     carve_slice_tables(a, p, L.tab);
-    carve_feeder(a, p, L.feed);
+    carve_feeder(a, p, L.feed, false);          // one batch holds every beam by default
     L.beams = a.take<int2>(n_beams);
 }
 
@@ -483,7 +483,7 @@ static void layout_multislice(Arena& a, const prism_params* p, MultisliceLayout&
     const int nb = prism_num_bins(p);
     L.batch = default_probe_batch(p, npix * 12);
     carve_slice_tables(a, p, L.tab);
-    carve_feeder(a, p, L.feed);
+    carve_feeder(a, p, L.feed, true);
     L.aperture_t = a.take<float2>(npix);
     L.phase_x = a.take<float2>((size_t)p->probes_x * p->nx);
     L.phase_y = a.take<float2>((size_t)p->probes_y * p->ny);
