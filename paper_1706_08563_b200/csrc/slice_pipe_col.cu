@@ -1,27 +1,20 @@
-// slice_pipe_col.cu -- software-pipelined forms of the two slice-step passes (grids of 256 .. 2048).
+// slice_pipe_col.cu -- software-pipelined column pass of the slice step (columns of 256 .. 1024 points).
 //
-// PAPER.md:44 Eq. (1)  psi <- psi * exp(i sigma V)          (transmission)
 // PAPER.md:80 Eq. (2)  Psi <- Psi * exp(-i pi lambda q^2 t)  (propagation), "done in Fourier space"
 //
-// Same arithmetic and the same two-pass structure as slice_pass.cu (row pass IFFT_x . t . FFT_x,
-// column pass FFT_y . P . IFFT_y, wave kept in mixed space A[w][y][kx] between them), organised so
-// that HBM transfers, shared-memory exchanges and butterflies of different lines overlap:
+// Column pass FFT_y . P . IFFT_y on mixed space A[w][y][kx] (see slice_pass.cu for the two-pass structure):
 //
-//  * every thread holds E = 32 points, so lines up to 1024 points need ONE shared-memory exchange
-//    per transform (2048: two) and inter-stage twiddles come from a transposed shared table;
-//  * row pass: a team (one warp; two for 2048-point lines) owns a private two-slot ring that the
-//    TMA engine fills with 1-D bulk copies (cp.async.bulk + mbarrier transaction counts); the slot
-//    the line lands in is also its exchange space; results go straight from registers to HBM.
-//    There is no CTA-wide barrier in the loop;
-//  * column pass: two teams of 256 threads per CTA alternate over [N rows] x [W columns] tiles of
-//    8192 points held in a three-buffer ring filled by 16-byte cp.async copies that signal an
-//    mbarrier; a lane owns one column of the tile and consecutive lanes consecutive columns, so every
-//    shared-memory access of the transforms is a contiguous run and results are stored from
-//    registers as 64-byte (W = 8) row segments;
+//  * every thread holds E = 32 points, so columns up to 1024 points need ONE shared-memory exchange
+//    per transform, and inter-stage twiddles come from a transposed shared table;
+//  * two teams of 256 threads per CTA alternate over [N rows] x [W columns] tiles of 8192 points held
+//    in a three-buffer ring filled by 16-byte cp.async copies that signal an mbarrier; a lane owns one
+//    column of the tile and consecutive lanes consecutive columns, so every shared-memory access of
+//    the transforms is a contiguous run and results are stored from registers as 64-byte (W = 8)
+//    row segments;
 //  * band-limit: after the column pass everything with |kx| > kx_max is exactly zero (2/3 rule,
-//    BASELINE.json), so mixed space is only ever read and written for kx in [0, xband) and
-//    [nx - xband, nx): the column pass runs on 2 xband / W tiles per wave and the row pass moves
-//    2 xband of the nx points of a line.
+//    BASELINE.json), so the pass runs on the 2 xband / W in-band tiles of a wave only.
+//
+// 2048-point columns run on the packed kernels of slice_pk.cu.
 #include "fft_core.cuh"
 #include "pipe_plan.cuh"
 #include "prism_internal.h"

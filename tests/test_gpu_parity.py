@@ -148,7 +148,7 @@ def _large_cases():
         # 1024^2 (one-exchange 32 x 32 transform), f=8 -> 128^2 windows, the grid of BASELINE.json config 4
         "T1024f8": W.scaled_test_case(1024, 3, 8, 4, voltage=200e3, alpha_mrad=12.0, defocus=50.0, seed_index=21,
                                       density=0.01),
-        # 2048^2 (32 x 16 x 4 transform), f=16 -> 128^2 windows, the grid of config 5; small aperture keeps
+        # 2048^2 (packed two-way transform, slice_pk.cu), f=16 -> 128^2 windows, the grid of config 5; small aperture keeps
         # the S-matrix of the test at a few GiB
         "T2048f16": W.scaled_test_case(2048, 2, 16, 4, voltage=300e3, alpha_mrad=6.0, seed_index=22,
                                        density=0.004),
@@ -196,6 +196,12 @@ def _odd_grid_cases():
         "R256x512": base.with_(name="R256x512", ny=512, cell=(25.6, 51.2, lz), probe_step=(6.4, 12.8)),
         # 0.1 x 0.2 Angstrom pixels: the band-limit circle is narrower than the default column band in kx
         "A256": base.with_(name="A256", cell=(25.6, 51.2, lz), probe_step=(6.4, 12.8), alpha=8e-3),
+        # 2048-point rows / columns on the packed kernels with the other axis short: run-time row stride, ragged
+        # line counts, and (anisotropic pixels) a band that is not the compile-time default
+        "R2048x256": base.with_(name="R2048x256", f=16, nx=2048, cell=(204.8, 25.6, lz), probe_step=(51.2, 6.4), alpha=6e-3),
+        "R256x2048": base.with_(name="R256x2048", f=16, ny=2048, cell=(25.6, 204.8, lz), probe_step=(6.4, 51.2), alpha=6e-3),
+        "A2048x256": base.with_(name="A2048x256", f=16, nx=2048, cell=(204.8, 51.2, lz), probe_step=(51.2, 12.8), alpha=5e-3),
+        "A256x2048": base.with_(name="A256x2048", f=16, ny=2048, cell=(51.2, 204.8, lz), probe_step=(12.8, 51.2), alpha=5e-3),
     }
 
 
