@@ -42,7 +42,11 @@ struct ColCfg {
     static constexpr int NBUF_FIT = (PIPE_SMEM_MAX - PIPE_HEADER - round_up_c(SmemTwiddles<P>::COUNT * 8, 128)) / (BUF * 8);
     static constexpr int NBUF = NBUF_FIT < NT + NT / 2 ? NBUF_FIT : NT + NT / 2;   // 3 buffers for 2 teams, 6 for 4
     static constexpr int TWB = round_up_c(SmemTwiddles<P>::COUNT * 8, 128);
-    static constexpr size_t SMEM = PIPE_HEADER + TWB + (size_t)NBUF * BUF * 8;
+    // the y-factor of the propagator sits in shared memory when it fits beside the tile ring (keeps 22 loads per
+    // thread and tile out of the LSU's global-memory queue)
+    static constexpr bool PY_SMEM = PIPE_HEADER + TWB + (size_t)NBUF * BUF * 8 + P::N * 8 <= PIPE_SMEM_MAX;
+    static constexpr int PYB = PY_SMEM ? P::N * 8 : 0;
+    static constexpr size_t SMEM = PIPE_HEADER + TWB + PYB + (size_t)NBUF * BUF * 8;
     static_assert(TEAM / 32 * LPW == P::T, "team shape");
     static_assert(SMEM <= PIPE_SMEM_MAX, "tile ring does not fit");
 };
@@ -71,11 +75,14 @@ __global__ void __launch_bounds__(ColCfg<P>::THREADS, 1) col_pipe_kernel(ColArgs
     extern __shared__ __align__(128) unsigned char smem_raw[];
     uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw);                    // [NBUF]
     float2* twtab = reinterpret_cast<float2*>(smem_raw + PIPE_HEADER);
-    float2* bufs = reinterpret_cast<float2*>(smem_raw + PIPE_HEADER + C::TWB);
+    float2* py_s = reinterpret_cast<float2*>(smem_raw + PIPE_HEADER + C::TWB);
+    float2* bufs = reinterpret_cast<float2*>(smem_raw + PIPE_HEADER + C::TWB + C::PYB);
     const int tid = threadIdx.x, tm = tid / C::TEAM, tt = tid % C::TEAM;
     const int lane = tt & 31, c = lane % W, t = (tt >> 5) * C::LPW + lane / W;
 
     SmemTwiddles<P>::fill(twtab, g.tw_y, tid, C::THREADS);
+    if (C::PY_SMEM && MODE != COL_MS_INIT)
+        for (int i = tid; i < N; i += C::THREADS) py_s[i] = __ldg(g.prop_y + i);
     if (LOADS && tid == 0) {
         for (int b = 0; b < C::NBUF; ++b) mbar_init(&full[b], C::TEAM);
         mbar_fence_init();
@@ -152,7 +159,7 @@ __global__ void __launch_bounds__(ColCfg<P>::THREADS, 1) col_pipe_kernel(ColArgs
                 if (YBE > 0 && e >= YBE && e < E - YBE) { v[e] = make_float2(0.f, 0.f); continue; }
                 const int m = t + T * e;
                 const int ky = e < E / 2 ? m : N - m;           // |ky|
-                const float2 pr = cmul(pxv, __ldg(g.prop_y + m));
+                const float2 pr = cmul(pxv, C::PY_SMEM ? py_s[m] : __ldg(g.prop_y + m));
                 v[e] = (ky <= lim) ? cmul(v[e], pr) : make_float2(0.f, 0.f);
             }
         }
