@@ -129,9 +129,9 @@ __global__ void __launch_bounds__(256, 2) lattice_dft_kernel(LatticeArgs g)
 #pragma unroll 8
             for (int c = c0; c < Q * Q; c += CPI) {
                 const int b = __ldg(g.cell_beam + c);
-                const float2 a = b >= 0 ? __ldg(g.coef + b) : make_float2(0.f, 0.f);
-                const float2 v = __ldg(src + (size_t)max(b, 0) * layer);
-                dst[(c / Q) * RS + (c % Q)] = cmul(a, v);
+                float2 r = make_float2(0.f, 0.f);           // residues no beam folds onto: no load
+                if (b >= 0) r = cmul(__ldg(g.coef + b), __ldg(src + (size_t)b * layer));
+                dst[(c / Q) * RS + (c % Q)] = r;
             }
         } else {
 #pragma unroll 2
