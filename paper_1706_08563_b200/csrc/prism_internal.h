@@ -29,7 +29,7 @@ struct RowArgs {
     float         scale;      // ROW_INIT: plane-wave amplitude; ROW_FINAL: output scale
 };
 cudaError_t launch_row_pass(RowMode mode, const RowArgs& args, cudaStream_t stream);
-// grids whose slice step runs on the pipelined kernels of slice_pipe.cu (both passes or neither)
+// grids whose slice step runs on the pipelined kernels of slice_pipe_row.cu / slice_pipe_col.cu or the packed ones of slice_pk.cu
 inline bool pipelined_grid(int nx, int ny) { return nx >= 256 && ny >= 256; }
 cudaError_t launch_row_pipe(RowMode mode, const RowArgs& args, cudaStream_t stream);
 // line lengths whose row pass runs on the packed-FFT kernels of slice_pk.cu; their transmission function is

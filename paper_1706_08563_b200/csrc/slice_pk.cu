@@ -4,7 +4,7 @@
 // PAPER.md:80 Eq. (2)  Psi <- Psi * exp(-i pi lambda q^2 t)  (propagation), "done in Fourier space"
 //
 // Same two passes, same mixed-space storage A[w][y][kx] and the same band-limit bookkeeping as
-// slice_pipe.cu; what changes is the transform: a line of N points is held by N / 64 threads (64 points
+// slice_pipe_row.cu / slice_pipe_col.cu; what changes is the transform: a line of N points is held by N / 64 threads (64 points
 // each), split by one radix-2 step in registers into two half-length transforms that run as the two
 // lanes of packed fp32 instructions, so a transform needs ONE shared-memory exchange up to 2048 points,
 // only warp-level barriers in the row pass, and about half the instructions per point:
