@@ -147,6 +147,36 @@ def oracle_sample(w, budget_s: float = 20.0):
     return n_probes / total, desc, cores, detail
 
 
+def run_reference_multislice(args, w):
+    """Oracle multislice on a bounded sample of MS2's probes (one per host thread), scaled linearly in probes."""
+    import oracle as O
+    cores = O.num_threads()
+    p = oracle_params(O, w)
+    lut_z, r_cut, lut_v = w.lut()
+    t0 = time.perf_counter()
+    v = O.potential(p, w.atoms_for_phonon(0), w.z, lut_z, r_cut, lut_v)
+    t_pot = time.perf_counter() - t0
+    xy = w.probe_xy()[:: max(1, w.n_probes // cores)][:cores]
+    vals = []
+    for i in range(args.warmup + args.steps):
+        t0 = time.perf_counter()
+        O.multislice_probes(p, v, xy)
+        dt = time.perf_counter() - t0
+        if i >= args.warmup:
+            vals.append(w.n_probes / (t_pot + dt * w.n_probes / len(xy)))
+    value = float(np.mean(vals))
+    desc = (f"oracle (fp64 C, gcc -O2, OpenMP x{cores}): whole potential, {len(xy)} of {w.n_probes} probes through "
+            f"{w.n_slices} slices, scaled linearly in probes")
+    print(json.dumps({
+        "impl": "reference", "metric": "multislice_probes_per_s", "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": len(vals), "warmup": args.warmup, "ms_per_step": 1e3 * w.n_probes / value, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"{w.name} ({WORKLOAD_NOTE.get(w.name, 'test case')}): plain multislice, {w.nx}x{w.ny}, "
+                               f"{w.n_slices} slices, {w.probes_x}x{w.probes_y} probes"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
+
+
 def run_reference(args):
     """--impl reference: the oracle is the reference arm for this tier (no pip-installable reference exists:
     /root/reference holds only the paper text)."""
@@ -155,6 +185,8 @@ def run_reference(args):
         return
     from paper_1706_08563_b200 import workloads
     w = workloads.get(args.workload)
+    if args.workload == "MS2":
+        return run_reference_multislice(args, w)
     vals, last = [], None
     t_begin = time.perf_counter()
     for i in range(args.warmup + args.steps):
@@ -190,6 +222,94 @@ def workload_config(w, args):
                   if w.nx >= 512 else "working set fits L2; L2 flushed between steps by the workspace writes"}
 
 
+
+# ------------------------------------------------------------------------------------------------ multislice line
+def run_multislice(args):
+    """--workload MS2 (BASELINE.json configs[1], the comparison path): a step is prism_build_potential ->
+    multislice_compute_output over the whole probe grid in the configuration's batches of 64 probes.  Reported as
+    multislice probes/s; one GPU only (the default PRISM line is the one the driver reads)."""
+    import torch
+    from paper_1706_08563_b200 import prism, workloads
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    dev = torch.device("cuda", int(os.environ.get("LOCAL_RANK", "0")))
+    torch.cuda.set_device(dev)
+    w = workloads.get(args.workload)
+    p = prism.params_from_workload(w)
+    lut_z, r_cut, lut_v = w.lut()
+    atoms = np.ascontiguousarray(w.atoms_for_phonon(0))
+    n_bins, n_probes, npix = prism.num_bins(p), w.n_probes, w.nx * w.ny
+    v = torch.empty((w.n_slices, w.ny, w.nx), dtype=torch.float32, device=dev)
+    out_dev = torch.empty((w.probes_y, w.probes_x, n_bins), dtype=torch.float32, device=dev)
+    out_host = torch.empty((w.probes_y, w.probes_x, n_bins), dtype=torch.float32).pin_memory()
+    ws = torch.empty(max(prism.workspace_bytes(p, prism.WS_POTENTIAL, len(w.z)),
+                         prism.workspace_bytes(p, prism.WS_MULTISLICE)), dtype=torch.uint8, device=dev)
+
+    def step(target):
+        prism.build_potential(p, atoms, w.z, lut_z, r_cut, lut_v, v, ws)
+        prism.multislice_output(p, v, target, ws)
+
+    for _ in range(args.warmup):
+        step(out_dev)
+    torch.cuda.synchronize()
+    sampler = ClockSampler(dev.index or 0)
+    sampler.start()
+    prism.launch_count(reset=True)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        step(out_dev)
+    e1.record()
+    torch.cuda.synchronize()
+    ms_per_step = e0.elapsed_time(e1) / args.steps
+    launches = prism.launch_count()
+    # per-kernel times come from a second, instrumented pass: this path is launch-bound (1700 launches of ~15 us per
+    # step) and a pair of events around every launch would slow the timed region itself by a quarter
+    prism.timing_enable(True)
+    for _ in range(args.steps):
+        step(out_dev)
+    torch.cuda.synchronize()
+    prism.timing_enable(False)
+    kern = prism.timing_read()
+    clocks = sampler.stop()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        step(out_host)
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    hbm_peak, peak_src = measured_peaks()
+    batch = w.batch if w.batch > 0 else n_probes
+    band = 2.0 * prism.band_columns(p) / w.nx if min(w.nx, w.ny) >= 256 else 1.0
+    per_launch = 16.0 * npix * band * min(batch, n_probes)              # one pass over one batch of probes
+    kernels = {}
+    for name, (ms, cnt) in kern.items():
+        entry = {"ms_per_step": ms / args.steps, "launches_per_step": cnt / args.steps, "avg_ms": ms / cnt}
+        if name in ("row_step", "col_step"):
+            entry["algorithmic_GBps"] = per_launch / (ms / cnt * 1e-3) / 1e9
+        kernels[name] = entry
+    top = max(kernels, key=lambda n: kernels[n]["ms_per_step"])
+    ach = kernels[top].get("algorithmic_GBps", 0.0)
+    line = {
+        "metric": "multislice_probes_per_s", "value": n_probes / (ms_per_step * 1e-3), "unit": UNIT, "n_gpus": 1,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "complex64", "data": "synthetic",
+        "config": {"workload": f"{w.name} ({WORKLOAD_NOTE.get(w.name, 'test case')}): {w.nx}x{w.ny} grid, {w.n_slices} slices, "
+                               f"{w.probes_x}x{w.probes_y} probes in batches of {batch}, {len(w.z)} atoms, plain multislice",
+                   "l2": "a batch of 64 waves (33.5 MB) fits L2; the three-batch rotation of the timed loop does not flush it"},
+        "clocks": clocks,
+        "e2e": {"value": n_probes * args.steps / e2e_s, "unit": UNIT,
+                "h2d_bytes_per_step": int(24 * len(w.z) + lut_v.size * 4 + 8 * (w.probes_x * w.nx + w.probes_y * w.ny + npix)),
+                "d2h_bytes_per_step": int(out_host.numel() * 4)},
+        "gpu_launches": int(launches),
+        "roofline": {"kernel": top, "bound": "hbm", "achieved": ach, "peak": hbm_peak, "unit": "GB/s",
+                     "frac": ach / hbm_peak, "traffic": None, "peak_source": peak_src, "bytes_per_launch": per_launch,
+                     "note": "launch-sized batches: the waves of a batch stay in L2, so this is not an HBM measurement"},
+        "kernels": kernels,
+    }
+    print(json.dumps(line))
+
 # ------------------------------------------------------------------------------------------------ CUDA arm
 def main():
     ap = argparse.ArgumentParser()
@@ -197,11 +317,13 @@ def main():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="P8", choices=["PR1", "P4", "P8", "P16"])
+    ap.add_argument("--workload", default="P8", choices=["PR1", "MS2", "P4", "P8", "P16"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.workload == "MS2":
+        return run_multislice(args)
 
     import torch
     from paper_1706_08563_b200 import prism, sharding, workloads
