@@ -35,6 +35,28 @@ __device__ __forceinline__ void cp_async_arrive(uint64_t* bar)
 __device__ __forceinline__ void named_barrier(int id, int nthreads)
 { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory"); }
 
+// ---- programmatic dependent launch (PDL) ------------------------------------------------------------------
+// The slice loop is a chain of kernels in one stream, each consuming what the previous one wrote.  Launched with
+// the programmatic-stream-serialization attribute, a kernel may start (run its prologue: tables into shared
+// memory, mbarrier init) while the previous one drains; griddep_wait() then blocks until the previous grid has
+// completed and its writes are visible.  Every kernel of the chain calls griddep_wait() before touching global
+// data and before griddep_launch(), so "the previous kernel has completed" still implies all earlier ones have.
+__device__ __forceinline__ void griddep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void griddep_launch() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
+template <class... KArgs, class... Args>
+inline cudaError_t launch_pdl(void (*kern)(KArgs...), unsigned grid, unsigned block, size_t smem, cudaStream_t stream,
+                              Args... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid); cfg.blockDim = dim3(block); cfg.dynamicSmemBytes = smem; cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
+}
+
 constexpr int PIPE_SMEM_MAX = 227 * 1024;
 constexpr int PIPE_HEADER = 1024;                     // mbarriers
 __host__ __device__ constexpr int round_up_c(int a, int b) { return (a + b - 1) / b * b; }

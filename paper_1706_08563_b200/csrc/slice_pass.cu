@@ -12,6 +12,7 @@
 // probe windows.
 #include "fft_core.cuh"
 #include "prism_internal.h"
+#include "pipe_ptx.cuh"
 
 namespace prism {
 
@@ -306,6 +307,8 @@ __global__ void transmission_kernel(const float* __restrict__ v, float2* __restr
 {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    griddep_wait();                          // part of the slice loop's chain of dependent launches (pipe_ptx.cuh)
+    griddep_launch();
     if (PAIRS) {
         for (; i < npix / 2; i += stride) {
             const float2 vv = reinterpret_cast<const float2*>(v)[i];
@@ -330,9 +333,8 @@ cudaError_t launch_transmission(const float* v, float2* t, double sigma, int64_t
     long long blocks = (npix + threads - 1) / threads;
     const long long cap = (long long)num_sms() * 8;
     if (blocks > cap) blocks = cap;
-    if (pairs) transmission_kernel<true><<<(unsigned)blocks, threads, 0, stream>>>(v, t, sigma, npix);
-    else transmission_kernel<false><<<(unsigned)blocks, threads, 0, stream>>>(v, t, sigma, npix);
-    return cudaGetLastError();
+    if (pairs) return launch_pdl(transmission_kernel<true>, (unsigned)blocks, threads, 0, stream, v, t, sigma, npix);
+    return launch_pdl(transmission_kernel<false>, (unsigned)blocks, threads, 0, stream, v, t, sigma, npix);
 }
 
 }  // namespace prism

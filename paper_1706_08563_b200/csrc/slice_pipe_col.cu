@@ -90,6 +90,8 @@ __global__ void __launch_bounds__(ColCfg<P>::THREADS, 1) col_pipe_kernel(ColArgs
     __syncthreads();
     SmemTwiddles<P> tw;
     tw.bind(twtab, t);
+    griddep_wait();                          // the previous kernel of the slice loop has completed (pipe_ptx.cuh)
+    griddep_launch();
 
     const int xb = g.xband;
     const int tiles_half = xb / W, tiles_per_wave = 2 * tiles_half;
@@ -200,8 +202,7 @@ static cudaError_t launch_col_pipe_s(const ColArgs& g, cudaStream_t stream)
     if (n_items == 0) return cudaSuccess;
     long long grid = (n_items + C::NT - 1) / C::NT;                 // at least one tile per team
     if (grid > num_sms()) grid = num_sms();
-    kern<<<(unsigned)grid, C::THREADS, C::SMEM, stream>>>(g);
-    return cudaGetLastError();
+    return launch_pdl(kern, (unsigned)grid, C::THREADS, C::SMEM, stream, g);
 }
 
 template <class P, int MODE>

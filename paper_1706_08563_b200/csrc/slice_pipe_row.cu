@@ -88,6 +88,8 @@ __global__ void __launch_bounds__(RowCfg<P, XBE>::THREADS, 1) row_pipe_kernel(Ro
     __syncthreads();
     SmemTwiddles<P> tw;
     tw.bind(twtab, t);
+    griddep_wait();                          // the previous kernel of the slice loop has completed (pipe_ptx.cuh)
+    griddep_launch();
 
     const long long n_lines = (long long)g.n_waves * g.ny;
     const long long n_groups = (n_lines + C::LPT - 1) / C::LPT;
@@ -194,8 +196,7 @@ static cudaError_t launch_row_pipe_x(const RowArgs& g, cudaStream_t stream)
     if (n_groups == 0) return cudaSuccess;
     long long grid = (n_groups + C::TEAMS - 1) / C::TEAMS;
     if (grid > num_sms()) grid = num_sms();
-    kern<<<(unsigned)grid, C::THREADS, C::SMEM, stream>>>(g);
-    return cudaGetLastError();
+    return launch_pdl(kern, (unsigned)grid, C::THREADS, C::SMEM, stream, g);
 }
 
 

@@ -65,6 +65,8 @@ __global__ void __launch_bounds__(RowPkCfg<N, XBE>::THREADS, 1) row_pk_kernel(Ro
     pk::fill_tables<P>(tab, g.tw_x, tid, C::THREADS);
     if (MODE != ROW_INIT && lane == 0) { mbar_init(&bars[warp], 1); mbar_fence_init(); }
     __syncthreads();
+    griddep_wait();                          // the previous kernel of the slice loop has completed (pipe_ptx.cuh)
+    griddep_launch();
 
     const long long n_lines = (long long)g.n_waves * g.ny;
     const long long n_groups = (n_lines + LPW - 1) / LPW;
@@ -192,8 +194,7 @@ static cudaError_t launch_row_pk_x(const RowArgs& g, cudaStream_t stream)
     if (n_groups == 0) return cudaSuccess;
     long long grid = (n_groups + C::WARPS - 1) / C::WARPS;
     if (grid > num_sms()) grid = num_sms();
-    kern<<<(unsigned)grid, C::THREADS, C::SMEM, stream>>>(g);
-    return cudaGetLastError();
+    return launch_pdl(kern, (unsigned)grid, C::THREADS, C::SMEM, stream, g);
 }
 
 template <int N, int MODE>
@@ -270,6 +271,8 @@ __global__ void __launch_bounds__(ColPkCfg<N>::THREADS, 1) col_pk_kernel(ColArgs
         mbar_fence_init();
     }
     __syncthreads();
+    griddep_wait();                          // the previous kernel of the slice loop has completed (pipe_ptx.cuh)
+    griddep_launch();
 
     const int xb = g.xband;
     const int tiles_half = xb / W, tiles_per_wave = 2 * tiles_half;
@@ -393,8 +396,7 @@ static cudaError_t launch_col_pk_s(const ColArgs& g, cudaStream_t stream)
     if (n_items == 0) return cudaSuccess;
     long long grid = (n_items + 1) / 2;                             // at least one tile per team
     if (grid > num_sms()) grid = num_sms();
-    kern<<<(unsigned)grid, C::THREADS, C::SMEM, stream>>>(g);
-    return cudaGetLastError();
+    return launch_pdl(kern, (unsigned)grid, C::THREADS, C::SMEM, stream, g);
 }
 
 template <int N, int MODE>
