@@ -325,3 +325,20 @@ def test_error_codes(G):
     with pytest.raises(prism.PrismError) as e:
         prism.build_potential(p, [[1.0, 1.0, 1.0]], [13], lut_z, r_cut, lut_v, v, G.ws(p, prism.WS_POTENTIAL, 1))
     assert e.value.code == prism.PRISM_ENOLUT
+
+
+def test_repeated_calls_are_bitwise_identical(G):
+    """The path has no atomics and a fixed summation order, and the slice loop's kernels are chained by programmatic
+    dependent launches: a missing dependency would show up as run-to-run differences."""
+    cases = [CASES["T512f8"], LARGE["T1024f8"], ODD["R2048x256"], ODD["A256x2048"]]
+    for w in cases:
+        v = G.gpu_potential(w)
+        assert torch.equal(v, G.gpu_potential(w))
+        s0, beams = G.gpu_smatrix(w, v)
+        out0 = G.gpu_prism_output(w, s0, beams)
+        m0 = G.gpu_multislice(w, v)
+        for _ in range(3):
+            s1, _ = G.gpu_smatrix(w, v)
+            assert torch.equal(s0, s1), w.name
+            assert np.array_equal(out0, G.gpu_prism_output(w, s1, beams)), w.name
+            assert np.array_equal(m0, G.gpu_multislice(w, v)), w.name
