@@ -8,6 +8,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <memory>
 #include <vector>
 
 #include "../../include/prism.h"
@@ -252,6 +253,30 @@ static cudaError_t upload(T* dst, const std::vector<T>& src, cudaStream_t st)
     return cudaMemcpyAsync(dst, src.data(), src.size() * sizeof(T), cudaMemcpyHostToDevice, st);
 }
 
+// Host tables are built first and uploaded together afterwards: an upload from pageable memory waits for the work
+// already queued on the stream, so interleaving "build a table, upload it" would leave the GPU idle while the
+// host builds the next one.  With the uploads deferred, the table building of a call overlaps the kernels the
+// previous call left running.
+struct DeferredUploads {
+    struct Item { void* dst; const void* src; size_t bytes; std::shared_ptr<void> keep; };
+    std::vector<Item> items;
+    template <class T> void add(T* dst, std::vector<T>&& src)
+    {
+        if (src.empty()) return;
+        auto keep = std::make_shared<std::vector<T>>(std::move(src));
+        items.push_back({dst, keep->data(), keep->size() * sizeof(T), keep});
+    }
+    template <class T> void add(T* dst, const std::vector<T>& src) { add(dst, std::vector<T>(src)); }
+    cudaError_t flush(cudaStream_t st)
+    {
+        for (const Item& it : items) {
+            cudaError_t e = cudaMemcpyAsync(it.dst, it.src, it.bytes, cudaMemcpyHostToDevice, st);
+            if (e != cudaSuccess) return e;
+        }
+        return cudaSuccess;
+    }
+};
+
 static int default_probe_batch(const prism_params* p, size_t bytes_per_probe)
 {
     long long n = (long long)p->probes_x * p->probes_y;
@@ -356,24 +381,23 @@ static void carve_slice_tables(Arena& a, const prism_params* p, SliceTables& t)
     t.prop_y = a.take<float2>(p->ny);
     t.ky_lim = a.take<int>(p->nx);
 }
-static int fill_slice_tables(const prism_params* p, const SliceTables& t, cudaStream_t st)
+static void fill_slice_tables(const prism_params* p, const SliceTables& t, DeferredUploads& up)
 {
     double lambda;
     electron_constants(p->voltage, &lambda, nullptr);
     std::vector<float2> h;
     twiddle_table(p->nx, h);
-    CU(upload(t.tw_x, h, st));
+    up.add(t.tw_x, std::move(h));
     twiddle_table(p->ny, h);
-    CU(upload(t.tw_y, h, st));
+    up.add(t.tw_y, std::move(h));
     // the row pass runs unscaled inverse FFTs and so does the column pass: fold 1/nx and 1/ny here
     propagator_factor(p->nx, p->cell[0], lambda, p->slice_thickness, 1.0 / p->nx, h);
-    CU(upload(t.prop_x, h, st));
+    up.add(t.prop_x, std::move(h));
     propagator_factor(p->ny, p->cell[1], lambda, p->slice_thickness, 1.0 / p->ny, h);
-    CU(upload(t.prop_y, h, st));
+    up.add(t.prop_y, std::move(h));
     std::vector<int> lim;
     band_limit(p, lim);
-    CU(upload(t.ky_lim, lim, st));
-    return PRISM_OK;
+    up.add(t.ky_lim, std::move(lim));
 }
 static void carve_feeder(Arena& a, const prism_params* p, SliceFeeder& f, bool many_batches)
 {
@@ -702,6 +726,7 @@ int prism_build_potential(const prism_params* p, const double* atoms_xyz, const 
     CU(upload(L.lut_v, h_lut, st));
     CU(upload(L.lut_rcut, h_rcut, st));
     CU(upload(d_atoms, sorted, st));
+    CU(cudaStreamSynchronize(st));          // the sorted host vectors are local; the kernels below run asynchronously
 
     PotentialArgs g;
     g.atoms = d_atoms; g.cell_start = L.cell_start; g.lut_v = L.lut_v; g.lut_rcut = L.lut_rcut; g.lut_n = lut_n;
@@ -724,8 +749,6 @@ int prism_build_potential(const prism_params* p, const double* atoms_xyz, const 
                                cudaMemcpyDeviceToHost, st));
         }
     }
-    // the sorted host vectors die here: make sure the (pageable) uploads have been staged
-    CU(cudaStreamSynchronize(st));
     return PRISM_OK;
 }
 
@@ -749,9 +772,12 @@ int prism_compute_smatrix(const prism_params* p, const float* v, int32_t* beams_
     SmatrixLayout L;
     layout_smatrix(a, p, n_beams, L);
     if (!a.ok()) return PRISM_ENOMEM;
-    if ((rc = fill_slice_tables(p, L.tab, st))) return rc;
+    DeferredUploads up;
+    fill_slice_tables(p, L.tab, up);
+    const int xband = band_columns(p), yband = band_rows(p);
+    CU(up.flush(st));
     CU(cudaMemcpyAsync(L.beams, beams.data(), beams.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
-    CU(cudaStreamSynchronize(st));          // `beams` (pageable) is local
+    CU(cudaStreamSynchronize(st));          // the host tables (pageable) are local
 
     double sigma;
     electron_constants(p->voltage, nullptr, &sigma);
@@ -762,7 +788,6 @@ int prism_compute_smatrix(const prism_params* p, const float* v, int32_t* beams_
     if ((rc = feed.init())) { feed.release(); return rc; }
 
     const int batch = p->batch > 0 ? std::min<int>(p->batch, n_beams) : n_beams;
-    const int xband = band_columns(p);
     auto run = [&]() -> int {
         for (int b0 = 0; b0 < n_beams; b0 += batch) {
             const int nb = std::min(batch, n_beams - b0);
@@ -772,7 +797,7 @@ int prism_compute_smatrix(const prism_params* p, const float* v, int32_t* beams_
             ra.n_waves = nb; ra.nx = p->nx; ra.ny = p->ny; ra.scale = 1.f; ra.xband = xband;
             ColArgs ca;
             std::memset(&ca, 0, sizeof(ca));
-            ca.xband = xband; ca.yband = band_rows(p);
+            ca.xband = xband; ca.yband = yband;
             ca.a = ra.a; ca.tw_y = L.tab.tw_y; ca.prop_x = L.tab.prop_x; ca.prop_y = L.tab.prop_y;
             ca.ky_lim = L.tab.ky_lim; ca.n_waves = nb; ca.nx = p->nx; ca.ny = p->ny; ca.scale = 1.f;
             feed.begin_sweep();
@@ -828,13 +853,14 @@ int prism_compute_output(const prism_params* p, const void* s, const int32_t* be
     const bool out_dev = pointer_is_device(out);
     float* d_out = out_dev ? out : L.out_stage;
 
-    // host tables (fp64)
+    // host tables (fp64), uploaded together below
+    DeferredUploads up;
     std::vector<float2> h;
     twiddle_table(mx, h);
-    CU(upload(L.tw_x, h, st));
+    up.add(L.tw_x, h);
     std::vector<float2> h2;
     twiddle_table(my, h2);
-    CU(upload(L.tw_y, h2, st));
+    up.add(L.tw_y, h2);
     std::vector<int> kxs(n_beams), kys(n_beams);
     std::vector<float2> coef(n_beams);
     const double wscale = 1.0 / (std::sqrt((double)n_beams) * std::sqrt((double)npix));     // R6
@@ -844,12 +870,12 @@ int prism_compute_output(const prism_params* p, const void* s, const int32_t* be
         const double chi = aberration(p, lambda, qx * qx + qy * qy);
         coef[b] = make_float2((float)(wscale * std::cos(-chi)), (float)(wscale * std::sin(-chi)));
     }
-    CU(upload(L.coef_b, coef, st));
+    up.add(L.coef_b, coef);
     std::vector<float2> phx, phy;
     position_phases(p->probes_x, p->probe_origin[0], p->probe_step[0], p->cell[0], kxs, phx);
     position_phases(p->probes_y, p->probe_origin[1], p->probe_step[1], p->cell[1], kys, phy);
-    CU(upload(L.phase_x, phx, st));
-    CU(upload(L.phase_y, phy, st));
+    up.add(L.phase_x, phx);
+    up.add(L.phase_y, phy);
     // window origin (R8): centre = round-half-up pixel, start = centre - M/2, periodic
     std::vector<int> wx0(p->probes_x), wy0(p->probes_y);
     const double px = p->cell[0] / p->nx, py = p->cell[1] / p->ny;
@@ -861,12 +887,12 @@ int prism_compute_output(const prism_params* p, const void* s, const int32_t* be
         const long long c = (long long)std::floor((p->probe_origin[1] + i * p->probe_step[1]) / py + 0.5);
         wy0[i] = (int)((((c - my / 2) % p->ny) + p->ny) % p->ny);
     }
-    CU(upload(L.win_x0, wx0, st));
-    CU(upload(L.win_y0, wy0, st));
+    up.add(L.win_x0, wx0);
+    up.add(L.win_y0, wy0);
     std::vector<int> bstart, bpix;
     ring_lists(p, mx, my, p->f, p->f, bstart, bpix);
-    CU(upload(L.bin_start, bstart, st));
-    CU(upload(L.bin_pix, bpix, st));
+    up.add(L.bin_start, bstart);
+    up.add(L.bin_pix, bpix);
     // regular probe lattice: the beam sum of all probes is a Q x Q DFT per S-matrix pixel
     LatticePlan lat = plan_lattice(p, beams, n_beams, wx0, wy0, mx, my);
     const int rows_per_batch = L.batch / p->probes_x;
@@ -881,9 +907,10 @@ int prism_compute_output(const prism_params* p, const void* s, const int32_t* be
             const double ang = -aberration(p, lambda, qx * qx + qy * qy) - 2.0 * kPi * turns;
             lcoef[b] = make_float2((float)(wscale * std::cos(ang)), (float)(wscale * std::sin(ang)));
         }
-        CU(upload(L.lat_coef, lcoef, st));
-        CU(upload(L.cell_beam, lat.cell_beam, st));
+        up.add(L.lat_coef, lcoef);
+        up.add(L.cell_beam, lat.cell_beam);
     }
+    CU(up.flush(st));
     CU(cudaStreamSynchronize(st));          // host vectors above are local
 
     const int n_probes = p->probes_x * p->probes_y;
@@ -944,7 +971,8 @@ int multislice_compute_output(const prism_params* p, const float* v, float* out,
     const bool out_dev = pointer_is_device(out);
     float* d_out = out_dev ? out : L.out_stage;
 
-    if ((rc = fill_slice_tables(p, L.tab, st))) return rc;
+    DeferredUploads up;
+    fill_slice_tables(p, L.tab, up);
     // probe spectrum (R4-R6): A_k exp(-i chi_k) * sqrt(nx ny) / sqrt(N_A), with the 1/ny of the
     // unscaled inverse column transform folded in; stored transposed [kx][ky]
     std::vector<float2> ap(npix, make_float2(0.f, 0.f));
@@ -966,19 +994,20 @@ int multislice_compute_output(const prism_params* p, const float* v, float* out,
                 ap[(size_t)sx * ny + sy] = make_float2((float)(amp * std::cos(-chi)), (float)(amp * std::sin(-chi)));
             }
         }
-    CU(upload(L.aperture_t, ap, st));
+    up.add(L.aperture_t, ap);
     std::vector<int> kxs(nx), kys(ny);
     for (int m = 0; m < nx; ++m) kxs[m] = signed_freq(m, nx);
     for (int m = 0; m < ny; ++m) kys[m] = signed_freq(m, ny);
     std::vector<float2> phx, phy;
     position_phases(p->probes_x, p->probe_origin[0], p->probe_step[0], p->cell[0], kxs, phx);
     position_phases(p->probes_y, p->probe_origin[1], p->probe_step[1], p->cell[1], kys, phy);
-    CU(upload(L.phase_x, phx, st));
-    CU(upload(L.phase_y, phy, st));
+    up.add(L.phase_x, phx);
+    up.add(L.phase_y, phy);
     std::vector<int> bstart, bpix;
     ring_lists(p, nx, ny, 1, 1, bstart, bpix);
-    CU(upload(L.bin_start, bstart, st));
-    CU(upload(L.bin_pix, bpix, st));
+    up.add(L.bin_start, bstart);
+    up.add(L.bin_pix, bpix);
+    CU(up.flush(st));
     CU(cudaStreamSynchronize(st));
 
     SliceFeeder& feed = L.feed;
