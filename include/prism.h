@@ -129,6 +129,17 @@ int prism_compute_output(const prism_params* p, const void* s, const int32_t* be
 int multislice_compute_output(const prism_params* p, const float* v, float* out,
                               void* workspace, size_t workspace_bytes, void* cuda_stream);
 
+/* Full diffraction patterns, the paper's "4D output" (PAPER.md:82 "2D, 3D or 4D outputs", :90):
+ * the same path as prism_compute_output / multislice_compute_output up to |FFT2|^2, without the ring integration.
+ *   patterns OUT DEVICE fp32 [probes_y * probes_x][my][mx] (PRISM: mx = nx / f, my = ny / f, pattern pixel (ky, kx)
+ *            at frequency (kx f / lx, ky f / ly); multislice: mx = nx, my = ny), array slot m = signed frequency
+ *            index as for the DFT convention above; normalised like the ring output (a pattern sums to at most 1).
+ *   Rings of prism_compute_output are sums of these pixels.  workspace: PRISM_WS_OUTPUT / PRISM_WS_MULTISLICE. */
+int prism_compute_patterns(const prism_params* p, const void* s, const int32_t* beams, int32_t n_beams,
+                           float* patterns, void* workspace, size_t workspace_bytes, void* cuda_stream);
+int multislice_compute_patterns(const prism_params* p, const float* v, float* patterns,
+                                void* workspace, size_t workspace_bytes, void* cuda_stream);
+
 /* Text for an error code, and the message of the last CUDA failure seen by the calling thread. */
 const char* prism_strerror(int code);
 const char* prism_last_error(void);

@@ -34,10 +34,10 @@ static int cuda_fail(cudaError_t e, const char* what)
 // CUDA events around every launch, on the stream the kernel is launched on.
 enum KernelClass { K_POTENTIAL = 0, K_TRANSMISSION, K_ROW_INIT, K_ROW_STEP, K_ROW_FINAL, K_COL_STEP,
                    K_BEAM_SUM, K_WIN_ROW_FFT, K_WIN_COL_ABS2, K_BIN_REDUCE, K_COL_MS_INIT, K_COL_MS_FINAL,
-                   K_LATTICE_DFT, K_NUM_CLASSES };
+                   K_LATTICE_DFT, K_PATTERNS, K_NUM_CLASSES };
 static const char* const kClassNames[K_NUM_CLASSES] = {
     "potential", "transmission", "row_init", "row_step", "row_final", "col_step", "beam_sum",
-    "win_row_fft", "win_col_abs2", "bin_reduce", "col_ms_init", "col_ms_final", "lattice_dft" };
+    "win_row_fft", "win_col_abs2", "bin_reduce", "col_ms_init", "col_ms_final", "lattice_dft", "patterns" };
 struct TimedLaunch { int cls; cudaEvent_t e0, e1; };
 static bool g_timing = false;
 static std::vector<TimedLaunch> g_timed;
@@ -832,14 +832,17 @@ static int copy_out(const prism_params* p, float* out, float* stage, bool out_is
     return PRISM_OK;
 }
 
-int prism_compute_output(const prism_params* p, const void* s, const int32_t* beams, int32_t n_beams,
-                         float* out, void* workspace, size_t workspace_bytes, void* cuda_stream)
+// rings (out != nullptr) or full patterns (patterns != nullptr) of every probe; shared by prism_compute_output and
+// prism_compute_patterns
+static int prism_output_impl(const prism_params* p, const void* s, const int32_t* beams, int32_t n_beams,
+                             float* out, float* patterns, void* workspace, size_t workspace_bytes, void* cuda_stream)
 {
     int rc = check_common(p);
     if (rc) return rc;
     if ((rc = check_probe(p))) return rc;
     if ((rc = check_prism(p))) return rc;
-    if (!s || !beams || n_beams < 1 || !out || !workspace) return PRISM_EINVAL;
+    if (!s || !beams || n_beams < 1 || (!out && !patterns) || !workspace) return PRISM_EINVAL;
+    if (patterns && !pointer_is_device(patterns)) return PRISM_EINVAL;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const int mx = p->nx / p->f, my = p->ny / p->f, nb = prism_num_bins(p);
     const size_t npix = (size_t)mx * my;
@@ -850,7 +853,7 @@ int prism_compute_output(const prism_params* p, const void* s, const int32_t* be
     OutputLayout L;
     layout_output(a, p, n_beams, L);
     if (!a.ok()) return PRISM_ENOMEM;
-    const bool out_dev = pointer_is_device(out);
+    const bool out_dev = out ? pointer_is_device(out) : true;
     float* d_out = out_dev ? out : L.out_stage;
 
     // host tables (fp64), uploaded together below
@@ -944,20 +947,38 @@ int prism_compute_output(const prism_params* p, const void* s, const int32_t* be
         ca.a = L.w; ca.intensity = L.intensity; ca.tw_y = L.tw_y; ca.n_waves = np; ca.nx = mx; ca.ny = my;
         ca.scale = (float)(1.0 / (double)npix);
         LAUNCH(K_WIN_COL_ABS2, launch_col_pass(COL_ABS2, ca, st), st);
-        LAUNCH(K_BIN_REDUCE, launch_bin_reduce(L.intensity, (int64_t)npix, L.bin_start, L.bin_pix, nb,
-                                 d_out + (size_t)p0 * nb, np, st), st);
+        if (patterns)
+            LAUNCH(K_PATTERNS, launch_transpose_patterns(L.intensity, patterns + (size_t)p0 * npix, mx, my, np, st), st);
+        if (out)
+            LAUNCH(K_BIN_REDUCE, launch_bin_reduce(L.intensity, (int64_t)npix, L.bin_start, L.bin_pix, nb,
+                                     d_out + (size_t)p0 * nb, np, st), st);
     }
-    return copy_out(p, out, L.out_stage, out_dev, st);
+    return out ? copy_out(p, out, L.out_stage, out_dev, st) : PRISM_OK;
+}
+
+int prism_compute_output(const prism_params* p, const void* s, const int32_t* beams, int32_t n_beams,
+                         float* out, void* workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    if (!out) return PRISM_EINVAL;
+    return prism_output_impl(p, s, beams, n_beams, out, nullptr, workspace, workspace_bytes, cuda_stream);
+}
+
+int prism_compute_patterns(const prism_params* p, const void* s, const int32_t* beams, int32_t n_beams,
+                           float* patterns, void* workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    if (!patterns) return PRISM_EINVAL;
+    return prism_output_impl(p, s, beams, n_beams, nullptr, patterns, workspace, workspace_bytes, cuda_stream);
 }
 
 // ---------------------------------------------------------------------------------------------------------
-int multislice_compute_output(const prism_params* p, const float* v, float* out,
-                              void* workspace, size_t workspace_bytes, void* cuda_stream)
+static int multislice_impl(const prism_params* p, const float* v, float* out, float* patterns,
+                           void* workspace, size_t workspace_bytes, void* cuda_stream)
 {
     int rc = check_common(p);
     if (rc) return rc;
     if ((rc = check_probe(p))) return rc;
-    if (!v || !out || !workspace) return PRISM_EINVAL;
+    if (!v || (!out && !patterns) || !workspace) return PRISM_EINVAL;
+    if (patterns && !pointer_is_device(patterns)) return PRISM_EINVAL;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const int nx = p->nx, ny = p->ny, nb = prism_num_bins(p);
     const size_t npix = (size_t)nx * ny;
@@ -968,7 +989,7 @@ int multislice_compute_output(const prism_params* p, const float* v, float* out,
     MultisliceLayout L;
     layout_multislice(a, p, L);
     if (!a.ok()) return PRISM_ENOMEM;
-    const bool out_dev = pointer_is_device(out);
+    const bool out_dev = out ? pointer_is_device(out) : true;
     float* d_out = out_dev ? out : L.out_stage;
 
     DeferredUploads up;
@@ -1044,15 +1065,32 @@ int multislice_compute_output(const prism_params* p, const float* v, float* out,
                 if (sl == p->n_slices - 1) LAUNCH(K_COL_MS_FINAL, launch_col_pass(COL_MS_FINAL, ca, st), st);
                 else LAUNCH(K_COL_STEP, launch_col_pass(COL_STEP, ca, st), st);
             }
-            LAUNCH(K_BIN_REDUCE, launch_bin_reduce(L.intensity, (int64_t)npix, L.bin_start, L.bin_pix, nb,
-                                     d_out + (size_t)p0 * nb, np, st), st);
+            if (patterns)
+                LAUNCH(K_PATTERNS, launch_transpose_patterns(L.intensity, patterns + (size_t)p0 * npix, nx, ny, np, st), st);
+            if (out)
+                LAUNCH(K_BIN_REDUCE, launch_bin_reduce(L.intensity, (int64_t)npix, L.bin_start, L.bin_pix, nb,
+                                         d_out + (size_t)p0 * nb, np, st), st);
         }
         return PRISM_OK;
     };
     rc = run();
     feed.release();
     if (rc) return rc;
-    return copy_out(p, out, L.out_stage, out_dev, st);
+    return out ? copy_out(p, out, L.out_stage, out_dev, st) : PRISM_OK;
+}
+
+int multislice_compute_output(const prism_params* p, const float* v, float* out,
+                              void* workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    if (!out) return PRISM_EINVAL;
+    return multislice_impl(p, v, out, nullptr, workspace, workspace_bytes, cuda_stream);
+}
+
+int multislice_compute_patterns(const prism_params* p, const float* v, float* patterns,
+                                void* workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    if (!patterns) return PRISM_EINVAL;
+    return multislice_impl(p, v, nullptr, patterns, workspace, workspace_bytes, cuda_stream);
 }
 
 #pragma GCC visibility pop

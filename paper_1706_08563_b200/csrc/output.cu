@@ -252,4 +252,44 @@ cudaError_t launch_bin_reduce(const float* intensity, int64_t npix, const int* b
     return cudaGetLastError();
 }
 
+
+// 4-D output: one pattern per probe in natural order.  32 x 32 tiles through padded shared memory,
+// coalesced on both sides.
+__global__ void __launch_bounds__(256) transpose_patterns_kernel(const float* __restrict__ in, float* __restrict__ out,
+                                                                 int mx, int my)
+{
+    __shared__ float tile[32][33];
+    const size_t npix = (size_t)mx * my;
+    const float* src = in + (size_t)blockIdx.z * npix;       // [kx][ky]
+    float* dst = out + (size_t)blockIdx.z * npix;            // [ky][kx]
+    const int ky0 = blockIdx.x * 32, kx0 = blockIdx.y * 32;
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;  // 32 x 8
+#pragma unroll
+    for (int r = ty; r < 32; r += 8) {
+        const int kx = kx0 + r, ky = ky0 + tx;
+        if (kx < mx && ky < my) tile[r][tx] = src[(size_t)kx * my + ky];
+    }
+    __syncthreads();
+#pragma unroll
+    for (int r = ty; r < 32; r += 8) {
+        const int ky = ky0 + r, kx = kx0 + tx;
+        if (kx < mx && ky < my) dst[(size_t)ky * mx + kx] = tile[tx][r];
+    }
+}
+
+cudaError_t launch_transpose_patterns(const float* intensity, float* patterns, int mx, int my, int n_waves,
+                                      cudaStream_t stream)
+{
+    if (n_waves == 0) return cudaSuccess;
+    for (int w0 = 0; w0 < n_waves; w0 += 65535) {             // gridDim.z limit
+        const int nw = n_waves - w0 < 65535 ? n_waves - w0 : 65535;
+        const dim3 grid((my + 31) / 32, (mx + 31) / 32, nw);
+        transpose_patterns_kernel<<<grid, 256, 0, stream>>>(intensity + (size_t)w0 * mx * my,
+                                                            patterns + (size_t)w0 * mx * my, mx, my);
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+    }
+    return cudaSuccess;
+}
+
 }  // namespace prism

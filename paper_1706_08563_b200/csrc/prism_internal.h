@@ -107,6 +107,11 @@ cudaError_t launch_bin_reduce(const float* intensity, int64_t npix, const int* b
                               const int* bin_pix, int n_bins, float* out, int n_waves,
                               cudaStream_t stream);
 
+// patterns[w][ky][kx] = intensity[w][kx][ky]: the column pass writes patterns transposed (ky contiguous), the 4-D
+// output wants them in natural order
+cudaError_t launch_transpose_patterns(const float* intensity, float* patterns, int mx, int my, int n_waves,
+                                      cudaStream_t stream);
+
 // ---- potential (potential.cu) ------------------------------------------------------
 struct PotAtom { double x, y; int32_t lut; int32_t pad; };
 struct PotentialArgs {

@@ -20,7 +20,7 @@ WS_SMATRIX, WS_OUTPUT, WS_MULTISLICE, WS_POTENTIAL = 0, 1, 2, 3
 
 EXPORTS = ["prism_workspace_bytes", "prism_num_bins", "prism_num_beams", "prism_band_columns", "prism_constants",
            "prism_build_potential", "prism_compute_smatrix", "prism_compute_output",
-           "multislice_compute_output", "prism_strerror", "prism_last_error", "prism_launch_count",
+           "multislice_compute_output", "prism_compute_patterns", "multislice_compute_patterns", "prism_strerror", "prism_last_error", "prism_launch_count",
            "prism_timing_enable", "prism_timing_classes", "prism_timing_class_name", "prism_timing_read"]
 
 
@@ -75,6 +75,10 @@ def _load() -> C.CDLL:
     lib.prism_compute_output.argtypes = [pp, vp, vp, i32, vp, vp, sz, vp]
     lib.multislice_compute_output.restype = C.c_int
     lib.multislice_compute_output.argtypes = [pp, vp, vp, vp, sz, vp]
+    lib.prism_compute_patterns.restype = C.c_int
+    lib.prism_compute_patterns.argtypes = [pp, vp, vp, i32, vp, vp, sz, vp]
+    lib.multislice_compute_patterns.restype = C.c_int
+    lib.multislice_compute_patterns.argtypes = [pp, vp, vp, vp, sz, vp]
     lib.prism_strerror.restype = C.c_char_p
     lib.prism_strerror.argtypes = [C.c_int]
     lib.prism_last_error.restype = C.c_char_p
@@ -209,3 +213,20 @@ def multislice_output(p: Params, v, out, workspace, stream=None):
                                           workspace.numel() * workspace.element_size(), _stream_ptr(stream)),
            "multislice_compute_output")
     return out
+
+
+def compute_patterns(p: Params, s, beams, patterns, workspace, stream=None):
+    """``prism_compute_patterns``.  ``patterns`` fp32 CUDA tensor ``[probes_y * probes_x][ny / f][nx / f]``."""
+    beams = np.ascontiguousarray(beams, dtype=np.int32).reshape(-1, 2)
+    _check(_lib.prism_compute_patterns(C.byref(p), _ptr(s), beams.ctypes.data, len(beams), _ptr(patterns),
+                                       _ptr(workspace), workspace.numel() * workspace.element_size(),
+                                       _stream_ptr(stream)), "prism_compute_patterns")
+    return patterns
+
+
+def multislice_patterns(p: Params, v, patterns, workspace, stream=None):
+    """``multislice_compute_patterns``.  ``patterns`` fp32 CUDA tensor ``[probes_y * probes_x][ny][nx]``."""
+    _check(_lib.multislice_compute_patterns(C.byref(p), _ptr(v), _ptr(patterns), _ptr(workspace),
+                                            workspace.numel() * workspace.element_size(), _stream_ptr(stream)),
+           "multislice_compute_patterns")
+    return patterns
