@@ -132,10 +132,13 @@ __global__ void __launch_bounds__(RowCfg<P, XBE>::THREADS, 1) row_pipe_kernel(Ro
             const int2 b = g.beams[w];
             const float2 wy = __ldg(g.tw_y + ((b.y * y) & (g.ny - 1)));
             const float2 base = make_float2(wy.x * g.scale, -wy.y * g.scale);
+            // exp(+2 pi i kx (t + T e) / N) = conj(w^(kx t)) conj(w^(kx T e)): one gathered table value per thread and
+            // one warp-uniform value per slot instead of E gathered loads
+            const float2 bt = cmul_conj(base, __ldg(g.tw_x + ((b.x * t) & (N - 1))));
 #pragma unroll
             for (int e = 0; e < E; ++e) {
-                const float2 wx = __ldg(g.tw_x + ((b.x * (t + T * e)) & (N - 1)));
-                v[e] = cmul_conj(base, wx);
+                const float2 we = __ldg(g.tw_x + ((b.x * T * e) & (N - 1)));
+                v[e] = cmul_conj(bt, we);
             }
         } else {
             mbar_wait(&bars[team], (unsigned)(it & 1));

@@ -136,12 +136,14 @@ __global__ void __launch_bounds__(RowPkCfg<N, XBE>::THREADS, 1) row_pk_kernel(Ro
                     const int2 b = g.beams[w];
                     const float2 wy = __ldg(g.tw_y + ((b.y * y) & (g.ny - 1)));
                     const float2 base = make_float2(wy.x * g.scale, -wy.y * g.scale);
+                    // x = 2 (t + T e) + {0, 1}: one gathered table value per thread and parity, one warp-uniform
+                    // value per slot (conj(w^(kx x)) = conj(w^(kx (2 t + h))) conj(w^(kx 2 T e)))
+                    const float2 b0 = cmul_conj(base, __ldg(g.tw_x + ((b.x * (2 * t)) & (N - 1))));
+                    const float2 b1 = cmul_conj(base, __ldg(g.tw_x + ((b.x * (2 * t + 1)) & (N - 1))));
 #pragma unroll
                     for (int e = 0; e < 32; ++e) {
-                        const int x0 = 2 * (t + T * e);
-                        const float2 w0 = __ldg(g.tw_x + ((b.x * x0) & (N - 1)));
-                        const float2 w1 = __ldg(g.tw_x + ((b.x * (x0 + 1)) & (N - 1)));
-                        const float2 v0 = cmul_conj(base, w0), v1 = cmul_conj(base, w1);
+                        const float2 we = __ldg(g.tw_x + ((b.x * (2 * T * e)) & (N - 1)));
+                        const float2 v0 = cmul_conj(b0, we), v1 = cmul_conj(b1, we);
                         p[e] = { make_float2(v0.x, v1.x), make_float2(v0.y, v1.y) };
                     }
                 } else {
