@@ -118,6 +118,30 @@ def test_p4_full(G):
     check_prism(G, W.p4(), n_layers=4, n_probes=12)
 
 
+def test_p4_full_patterns(G):
+    """4-D output at config 3's size (16384 patterns of 128^2): sampled patterns against the oracle's stage 2 applied
+    to the GPU S-matrix, pixel by pixel, and the rings as sums of their pixels."""
+    from paper_1706_08563_b200 import prism
+    w = W.p4()
+    p = oracle_params(w)
+    pp = prism.params_from_workload(w)
+    v = G.gpu_potential(w)
+    s, beams = G.gpu_smatrix(w, v)
+    m = w.nx // w.f
+    pat = torch.empty((w.n_probes, m, m), dtype=torch.float32, device=G.DEV)
+    prism.compute_patterns(pp, s, beams, pat, G.ws(pp, prism.WS_OUTPUT))
+    out = G.gpu_prism_output(w, s, beams)
+    s64 = s.cpu().numpy().astype(np.complex128)
+    xy = w.probe_xy()
+    for i in spread(len(xy), 6):
+        _, ref = O.prism_probe(p, s64, beams, xy[i, 0], xy[i, 1], want_pattern=True)
+        got = pat[i].cpu().numpy().astype(np.float64)
+        assert rel_l2(got, ref) < TOL_STAGE2, i
+        assert np.allclose(O.bin_intensity(p, got, w.f, w.f), out[i], rtol=1e-5, atol=1e-9)
+    tot = pat.sum(dim=(1, 2)).cpu().numpy()
+    assert np.all(tot > 0.5) and np.all(tot < 1.05)
+
+
 def test_p8_full(G):
     """BASELINE.json configs[3]: 1024^2, 50 slices, f = 8, 509 beams, 256 x 256 probes, defocus 50 A."""
     check_prism(G, W.p8(), n_layers=4, n_probes=12)
