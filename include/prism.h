@@ -140,6 +140,18 @@ int prism_compute_patterns(const prism_params* p, const void* s, const int32_t* 
 int multislice_compute_patterns(const prism_params* p, const float* v, float* patterns,
                                 void* workspace, size_t workspace_bytes, void* cuda_stream);
 
+/* Arbitrary virtual detectors ("the probe intensity is summed in Fourier space to determine the virtual
+ * detector signal"; one detector gives the paper's 2-D output): out[probe][d] = sum over the pattern pixels of
+ * masks[d][ky][kx] * I[ky][kx], with the patterns of prism_compute_patterns / multislice_compute_patterns.
+ *   masks IN  DEVICE fp32 [n_masks][my][mx] (weights; 0 / 1 for a plain detector), 1 <= n_masks <= 16
+ *   out   OUT DEVICE fp32 [probes_y * probes_x][n_masks]
+ * Fixed summation order (deterministic).  workspace: PRISM_WS_OUTPUT / PRISM_WS_MULTISLICE. */
+int prism_compute_detectors(const prism_params* p, const void* s, const int32_t* beams, int32_t n_beams,
+                            const float* masks, int32_t n_masks, float* out,
+                            void* workspace, size_t workspace_bytes, void* cuda_stream);
+int multislice_compute_detectors(const prism_params* p, const float* v, const float* masks, int32_t n_masks,
+                                 float* out, void* workspace, size_t workspace_bytes, void* cuda_stream);
+
 /* Text for an error code, and the message of the last CUDA failure seen by the calling thread. */
 const char* prism_strerror(int code);
 const char* prism_last_error(void);

@@ -34,10 +34,10 @@ static int cuda_fail(cudaError_t e, const char* what)
 // CUDA events around every launch, on the stream the kernel is launched on.
 enum KernelClass { K_POTENTIAL = 0, K_TRANSMISSION, K_ROW_INIT, K_ROW_STEP, K_ROW_FINAL, K_COL_STEP,
                    K_BEAM_SUM, K_WIN_ROW_FFT, K_WIN_COL_ABS2, K_BIN_REDUCE, K_COL_MS_INIT, K_COL_MS_FINAL,
-                   K_LATTICE_DFT, K_PATTERNS, K_NUM_CLASSES };
+                   K_LATTICE_DFT, K_PATTERNS, K_DETECTORS, K_NUM_CLASSES };
 static const char* const kClassNames[K_NUM_CLASSES] = {
     "potential", "transmission", "row_init", "row_step", "row_final", "col_step", "beam_sum",
-    "win_row_fft", "win_col_abs2", "bin_reduce", "col_ms_init", "col_ms_final", "lattice_dft", "patterns" };
+    "win_row_fft", "win_col_abs2", "bin_reduce", "col_ms_init", "col_ms_final", "lattice_dft", "patterns", "detectors" };
 struct TimedLaunch { int cls; cudaEvent_t e0, e1; };
 static bool g_timing = false;
 static std::vector<TimedLaunch> g_timed;
@@ -832,17 +832,30 @@ static int copy_out(const prism_params* p, float* out, float* stage, bool out_is
     return PRISM_OK;
 }
 
-// rings (out != nullptr) or full patterns (patterns != nullptr) of every probe; shared by prism_compute_output and
-// prism_compute_patterns
+// virtual detectors requested beside / instead of the rings: det[probe][d] = sum masks[d] * pattern
+struct DetectorRequest { const float* masks = nullptr; int n_masks = 0; float* out = nullptr; };
+static int check_detectors(const DetectorRequest& d)
+{
+    if (!d.out && !d.masks) return PRISM_OK;
+    if (!d.out || !d.masks || d.n_masks < 1) return PRISM_EINVAL;
+    if (d.n_masks > 16) return PRISM_EUNSUPPORTED;
+    if (!pointer_is_device(d.out) || !pointer_is_device(d.masks)) return PRISM_EINVAL;
+    return PRISM_OK;
+}
+
+// rings (out), full patterns (patterns) and / or virtual detectors (det) of every probe; shared by
+// prism_compute_output, prism_compute_patterns and prism_compute_detectors
 static int prism_output_impl(const prism_params* p, const void* s, const int32_t* beams, int32_t n_beams,
-                             float* out, float* patterns, void* workspace, size_t workspace_bytes, void* cuda_stream)
+                             float* out, float* patterns, const DetectorRequest& det,
+                             void* workspace, size_t workspace_bytes, void* cuda_stream)
 {
     int rc = check_common(p);
     if (rc) return rc;
     if ((rc = check_probe(p))) return rc;
     if ((rc = check_prism(p))) return rc;
-    if (!s || !beams || n_beams < 1 || (!out && !patterns) || !workspace) return PRISM_EINVAL;
+    if (!s || !beams || n_beams < 1 || (!out && !patterns && !det.out) || !workspace) return PRISM_EINVAL;
     if (patterns && !pointer_is_device(patterns)) return PRISM_EINVAL;
+    if ((rc = check_detectors(det))) return rc;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const int mx = p->nx / p->f, my = p->ny / p->f, nb = prism_num_bins(p);
     const size_t npix = (size_t)mx * my;
@@ -949,6 +962,9 @@ static int prism_output_impl(const prism_params* p, const void* s, const int32_t
         LAUNCH(K_WIN_COL_ABS2, launch_col_pass(COL_ABS2, ca, st), st);
         if (patterns)
             LAUNCH(K_PATTERNS, launch_transpose_patterns(L.intensity, patterns + (size_t)p0 * npix, mx, my, np, st), st);
+        if (det.out)
+            LAUNCH(K_DETECTORS, launch_mask_dot(L.intensity, det.masks, det.n_masks, mx, my,
+                                                det.out + (size_t)p0 * det.n_masks, np, st), st);
         if (out)
             LAUNCH(K_BIN_REDUCE, launch_bin_reduce(L.intensity, (int64_t)npix, L.bin_start, L.bin_pix, nb,
                                      d_out + (size_t)p0 * nb, np, st), st);
@@ -960,25 +976,36 @@ int prism_compute_output(const prism_params* p, const void* s, const int32_t* be
                          float* out, void* workspace, size_t workspace_bytes, void* cuda_stream)
 {
     if (!out) return PRISM_EINVAL;
-    return prism_output_impl(p, s, beams, n_beams, out, nullptr, workspace, workspace_bytes, cuda_stream);
+    return prism_output_impl(p, s, beams, n_beams, out, nullptr, DetectorRequest(), workspace, workspace_bytes, cuda_stream);
 }
 
 int prism_compute_patterns(const prism_params* p, const void* s, const int32_t* beams, int32_t n_beams,
                            float* patterns, void* workspace, size_t workspace_bytes, void* cuda_stream)
 {
     if (!patterns) return PRISM_EINVAL;
-    return prism_output_impl(p, s, beams, n_beams, nullptr, patterns, workspace, workspace_bytes, cuda_stream);
+    return prism_output_impl(p, s, beams, n_beams, nullptr, patterns, DetectorRequest(), workspace, workspace_bytes, cuda_stream);
+}
+
+int prism_compute_detectors(const prism_params* p, const void* s, const int32_t* beams, int32_t n_beams,
+                            const float* masks, int32_t n_masks, float* out,
+                            void* workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    if (!out || !masks) return PRISM_EINVAL;
+    DetectorRequest det;
+    det.masks = masks; det.n_masks = n_masks; det.out = out;
+    return prism_output_impl(p, s, beams, n_beams, nullptr, nullptr, det, workspace, workspace_bytes, cuda_stream);
 }
 
 // ---------------------------------------------------------------------------------------------------------
 static int multislice_impl(const prism_params* p, const float* v, float* out, float* patterns,
-                           void* workspace, size_t workspace_bytes, void* cuda_stream)
+                           const DetectorRequest& det, void* workspace, size_t workspace_bytes, void* cuda_stream)
 {
     int rc = check_common(p);
     if (rc) return rc;
     if ((rc = check_probe(p))) return rc;
-    if (!v || (!out && !patterns) || !workspace) return PRISM_EINVAL;
+    if (!v || (!out && !patterns && !det.out) || !workspace) return PRISM_EINVAL;
     if (patterns && !pointer_is_device(patterns)) return PRISM_EINVAL;
+    if ((rc = check_detectors(det))) return rc;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const int nx = p->nx, ny = p->ny, nb = prism_num_bins(p);
     const size_t npix = (size_t)nx * ny;
@@ -1067,6 +1094,9 @@ static int multislice_impl(const prism_params* p, const float* v, float* out, fl
             }
             if (patterns)
                 LAUNCH(K_PATTERNS, launch_transpose_patterns(L.intensity, patterns + (size_t)p0 * npix, nx, ny, np, st), st);
+            if (det.out)
+                LAUNCH(K_DETECTORS, launch_mask_dot(L.intensity, det.masks, det.n_masks, nx, ny,
+                                                    det.out + (size_t)p0 * det.n_masks, np, st), st);
             if (out)
                 LAUNCH(K_BIN_REDUCE, launch_bin_reduce(L.intensity, (int64_t)npix, L.bin_start, L.bin_pix, nb,
                                          d_out + (size_t)p0 * nb, np, st), st);
@@ -1083,14 +1113,23 @@ int multislice_compute_output(const prism_params* p, const float* v, float* out,
                               void* workspace, size_t workspace_bytes, void* cuda_stream)
 {
     if (!out) return PRISM_EINVAL;
-    return multislice_impl(p, v, out, nullptr, workspace, workspace_bytes, cuda_stream);
+    return multislice_impl(p, v, out, nullptr, DetectorRequest(), workspace, workspace_bytes, cuda_stream);
 }
 
 int multislice_compute_patterns(const prism_params* p, const float* v, float* patterns,
                                 void* workspace, size_t workspace_bytes, void* cuda_stream)
 {
     if (!patterns) return PRISM_EINVAL;
-    return multislice_impl(p, v, nullptr, patterns, workspace, workspace_bytes, cuda_stream);
+    return multislice_impl(p, v, nullptr, patterns, DetectorRequest(), workspace, workspace_bytes, cuda_stream);
+}
+
+int multislice_compute_detectors(const prism_params* p, const float* v, const float* masks, int32_t n_masks,
+                                 float* out, void* workspace, size_t workspace_bytes, void* cuda_stream)
+{
+    if (!out || !masks) return PRISM_EINVAL;
+    DetectorRequest det;
+    det.masks = masks; det.n_masks = n_masks; det.out = out;
+    return multislice_impl(p, v, nullptr, nullptr, det, workspace, workspace_bytes, cuda_stream);
 }
 
 #pragma GCC visibility pop

@@ -292,4 +292,68 @@ cudaError_t launch_transpose_patterns(const float* intensity, float* patterns, i
     return cudaSuccess;
 }
 
+// Arbitrary virtual detectors: out[w][d] = sum_pix masks[d][ky][kx] * intensity[w][kx][ky].  One CTA per
+// pattern walks 32 x 32 tiles: the intensity tile is read with ky contiguous, each mask tile with kx contiguous, and
+// they meet through a padded shared-memory tile.  Fixed summation order (deterministic).
+constexpr int MAX_MASKS = 16;
+template <int NM>                                        // NM >= n_masks: accumulators kept in registers
+__global__ void __launch_bounds__(256) mask_dot_kernel(const float* __restrict__ intensity, const float* __restrict__ masks,
+                                                       int n_masks, int mx, int my, float* __restrict__ out)
+{
+    __shared__ float tile[32][33];
+    __shared__ float part[8][NM];
+    const size_t npix = (size_t)mx * my;
+    const float* img = intensity + (size_t)blockIdx.x * npix;        // [kx][ky]
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+    float acc[NM];
+#pragma unroll
+    for (int d = 0; d < NM; ++d) acc[d] = 0.f;
+    for (int kx0 = 0; kx0 < mx; kx0 += 32)
+        for (int ky0 = 0; ky0 < my; ky0 += 32) {
+            __syncthreads();
+#pragma unroll
+            for (int r = ty; r < 32; r += 8) {
+                const int kx = kx0 + r, ky = ky0 + tx;
+                tile[r][tx] = (kx < mx && ky < my) ? img[(size_t)kx * my + ky] : 0.f;
+            }
+            __syncthreads();
+#pragma unroll
+            for (int r = ty; r < 32; r += 8) {
+                const int ky = ky0 + r, kx = kx0 + tx;
+                if (kx < mx && ky < my) {
+                    const float v = tile[tx][r];
+#pragma unroll
+                    for (int d = 0; d < NM; ++d)
+                        if (d < n_masks) acc[d] = fmaf(__ldg(masks + (size_t)d * npix + (size_t)ky * mx + kx), v, acc[d]);
+                }
+            }
+        }
+#pragma unroll
+    for (int d = 0; d < NM; ++d) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) acc[d] += __shfl_xor_sync(0xffffffffu, acc[d], o);
+        if (tx == 0) part[ty][d] = acc[d];
+    }
+    __syncthreads();
+    if (threadIdx.x < n_masks) {
+        float sum = 0.f;
+#pragma unroll
+        for (int w = 0; w < 8; ++w) sum += part[w][threadIdx.x];
+        out[(size_t)blockIdx.x * n_masks + threadIdx.x] = sum;
+    }
+}
+
+cudaError_t launch_mask_dot(const float* intensity, const float* masks, int n_masks, int mx, int my, float* out,
+                            int n_waves, cudaStream_t stream)
+{
+    if (n_waves == 0 || n_masks == 0) return cudaSuccess;
+    if (n_masks > MAX_MASKS) return cudaErrorInvalidValue;
+    if (n_masks <= 1)      mask_dot_kernel<1><<<n_waves, 256, 0, stream>>>(intensity, masks, n_masks, mx, my, out);
+    else if (n_masks <= 2) mask_dot_kernel<2><<<n_waves, 256, 0, stream>>>(intensity, masks, n_masks, mx, my, out);
+    else if (n_masks <= 4) mask_dot_kernel<4><<<n_waves, 256, 0, stream>>>(intensity, masks, n_masks, mx, my, out);
+    else if (n_masks <= 8) mask_dot_kernel<8><<<n_waves, 256, 0, stream>>>(intensity, masks, n_masks, mx, my, out);
+    else                   mask_dot_kernel<16><<<n_waves, 256, 0, stream>>>(intensity, masks, n_masks, mx, my, out);
+    return cudaGetLastError();
+}
+
 }  // namespace prism

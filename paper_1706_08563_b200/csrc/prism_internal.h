@@ -112,6 +112,10 @@ cudaError_t launch_bin_reduce(const float* intensity, int64_t npix, const int* b
 cudaError_t launch_transpose_patterns(const float* intensity, float* patterns, int mx, int my, int n_waves,
                                       cudaStream_t stream);
 
+// out[w][d] = sum over pixels of masks[d][ky][kx] * intensity[w][kx][ky], d < n_masks <= 16 (virtual detectors)
+cudaError_t launch_mask_dot(const float* intensity, const float* masks, int n_masks, int mx, int my, float* out,
+                            int n_waves, cudaStream_t stream);
+
 // ---- potential (potential.cu) ------------------------------------------------------
 struct PotAtom { double x, y; int32_t lut; int32_t pad; };
 struct PotentialArgs {

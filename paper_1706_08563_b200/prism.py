@@ -20,7 +20,8 @@ WS_SMATRIX, WS_OUTPUT, WS_MULTISLICE, WS_POTENTIAL = 0, 1, 2, 3
 
 EXPORTS = ["prism_workspace_bytes", "prism_num_bins", "prism_num_beams", "prism_band_columns", "prism_constants",
            "prism_build_potential", "prism_compute_smatrix", "prism_compute_output",
-           "multislice_compute_output", "prism_compute_patterns", "multislice_compute_patterns", "prism_strerror", "prism_last_error", "prism_launch_count",
+           "multislice_compute_output", "prism_compute_patterns", "multislice_compute_patterns",
+           "prism_compute_detectors", "multislice_compute_detectors", "prism_strerror", "prism_last_error", "prism_launch_count",
            "prism_timing_enable", "prism_timing_classes", "prism_timing_class_name", "prism_timing_read"]
 
 
@@ -79,6 +80,10 @@ def _load() -> C.CDLL:
     lib.prism_compute_patterns.argtypes = [pp, vp, vp, i32, vp, vp, sz, vp]
     lib.multislice_compute_patterns.restype = C.c_int
     lib.multislice_compute_patterns.argtypes = [pp, vp, vp, vp, sz, vp]
+    lib.prism_compute_detectors.restype = C.c_int
+    lib.prism_compute_detectors.argtypes = [pp, vp, vp, i32, vp, i32, vp, vp, sz, vp]
+    lib.multislice_compute_detectors.restype = C.c_int
+    lib.multislice_compute_detectors.argtypes = [pp, vp, vp, i32, vp, vp, sz, vp]
     lib.prism_strerror.restype = C.c_char_p
     lib.prism_strerror.argtypes = [C.c_int]
     lib.prism_last_error.restype = C.c_char_p
@@ -230,3 +235,22 @@ def multislice_patterns(p: Params, v, patterns, workspace, stream=None):
                                             workspace.numel() * workspace.element_size(), _stream_ptr(stream)),
            "multislice_compute_patterns")
     return patterns
+
+
+def compute_detectors(p: Params, s, beams, masks, out, workspace, stream=None):
+    """``prism_compute_detectors``.  ``masks`` fp32 CUDA ``[n_masks][ny / f][nx / f]``, ``out`` fp32 CUDA
+    ``[probes_y * probes_x][n_masks]``."""
+    beams = np.ascontiguousarray(beams, dtype=np.int32).reshape(-1, 2)
+    _check(_lib.prism_compute_detectors(C.byref(p), _ptr(s), beams.ctypes.data, len(beams), _ptr(masks),
+                                        int(masks.shape[0]), _ptr(out), _ptr(workspace),
+                                        workspace.numel() * workspace.element_size(), _stream_ptr(stream)),
+           "prism_compute_detectors")
+    return out
+
+
+def multislice_detectors(p: Params, v, masks, out, workspace, stream=None):
+    """``multislice_compute_detectors``.  ``masks`` fp32 CUDA ``[n_masks][ny][nx]``."""
+    _check(_lib.multislice_compute_detectors(C.byref(p), _ptr(v), _ptr(masks), int(masks.shape[0]), _ptr(out),
+                                             _ptr(workspace), workspace.numel() * workspace.element_size(),
+                                             _stream_ptr(stream)), "multislice_compute_detectors")
+    return out

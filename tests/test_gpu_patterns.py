@@ -112,3 +112,84 @@ def test_patterns_argument_checks(G):
     with pytest.raises(prism.PrismError) as e:
         prism.compute_patterns(p, s, beams, host, G.ws(p, prism.WS_OUTPUT))      # patterns must be device memory
     assert e.value.code == prism.PRISM_EINVAL
+
+
+# ---- arbitrary virtual detectors (2-D output = one detector) ---------------------------------------------------
+def _masks(w, p, my, mx, fy, fx, rng):
+    """An annular detector built from the oracle's own angle convention (rings 3..7 of bin_intensity), a random
+    weight mask, a half-plane (segmented) detector, and the all-ones mask."""
+    lam, _ = O.constants(w.voltage)
+    ky = np.where(np.arange(my) < my // 2, np.arange(my), np.arange(my) - my) * fy
+    kx = np.where(np.arange(mx) < mx // 2, np.arange(mx), np.arange(mx) - mx) * fx
+    ang = lam * np.sqrt((kx[None, :] / w.cell[0]) ** 2 + (ky[:, None] / w.cell[1]) ** 2)
+    ring = np.floor(ang / w.det_step)
+    annular = ((ring >= 3) & (ring < 8)).astype(np.float64)
+    return np.stack([annular, rng.random((my, mx)), (kx[None, :] > 0) * np.ones((my, 1)), np.ones((my, mx))])
+
+
+@pytest.mark.parametrize("name", ["PR1", "T128f2", "R2048x256"])
+def test_prism_detectors_parity(G, name):
+    from paper_1706_08563_b200 import prism
+    w = CASES[name]
+    p = oracle_params(w)
+    pp = prism.params_from_workload(w)
+    v = G.gpu_potential(w)
+    s, beams = G.gpu_smatrix(w, v)
+    my, mx = w.ny // w.f, w.nx // w.f
+    masks = _masks(w, p, my, mx, w.f, w.f, np.random.default_rng(5))
+    m_dev = torch.as_tensor(masks, dtype=torch.float32, device=G.DEV).contiguous()
+    out = torch.empty((w.n_probes, len(masks)), dtype=torch.float32, device=G.DEV)
+    prism.compute_detectors(pp, s, beams, m_dev, out, G.ws(pp, prism.WS_OUTPUT))
+    torch.cuda.synchronize()
+    got = out.cpu().numpy().astype(np.float64)
+    s_ref = O.smatrix(p, oracle_potential(w), beams)
+    xy = w.probe_xy()
+    m32 = m_dev.cpu().numpy().astype(np.float64)             # the weights the kernel saw
+    ref = np.empty_like(got)
+    for i in range(len(xy)):
+        bins, pat = O.prism_probe(p, s_ref, beams, xy[i, 0], xy[i, 1], want_pattern=True)
+        ref[i] = (m32 * pat[None]).sum(axis=(1, 2))
+        assert abs(ref[i, 0] - bins[3:8].sum()) < 1e-12          # the annular mask is rings 3..7 of the oracle
+        assert abs(ref[i, 3] - pat.sum()) < 1e-12
+    assert rel_l2(got, ref) < TOL
+    for d in range(len(masks)):
+        assert rel_l2(got[:, d], ref[:, d]) < 5 * TOL, d
+    # one annular detector = a sum of rings of the 3-D output
+    rings = G.gpu_prism_output(w, s, beams)
+    assert np.allclose(got[:, 0], rings[:, 3:8].sum(axis=1), rtol=1e-5, atol=1e-9)
+    # deterministic
+    out2 = torch.empty_like(out)
+    prism.compute_detectors(pp, s, beams, m_dev, out2, G.ws(pp, prism.WS_OUTPUT))
+    assert torch.equal(out, out2)
+
+
+def test_multislice_detectors_parity(G):
+    from paper_1706_08563_b200 import prism
+    w = CASES["L256f2q32"].with_(probes_x=3, probes_y=2)
+    p = oracle_params(w)
+    pp = prism.params_from_workload(w)
+    v = G.gpu_potential(w)
+    masks = _masks(w, p, w.ny, w.nx, 1, 1, np.random.default_rng(6))
+    m_dev = torch.as_tensor(masks, dtype=torch.float32, device=G.DEV).contiguous()
+    out = torch.empty((w.n_probes, len(masks)), dtype=torch.float32, device=G.DEV)
+    prism.multislice_detectors(pp, v, m_dev, out, G.ws(pp, prism.WS_MULTISLICE))
+    torch.cuda.synchronize()
+    got = out.cpu().numpy().astype(np.float64)
+    v_ref = oracle_potential(w)
+    m32 = m_dev.cpu().numpy().astype(np.float64)
+    ref = np.stack([(m32 * O.multislice_probe(p, v_ref, x, y, want_pattern=True)[1][None]).sum(axis=(1, 2))
+                    for x, y in w.probe_xy()])
+    assert rel_l2(got, ref) < TOL
+
+
+def test_detector_argument_checks(G):
+    from paper_1706_08563_b200 import prism
+    w = CASES["PR1"]
+    pp = prism.params_from_workload(w)
+    v = G.gpu_potential(w)
+    s, beams = G.gpu_smatrix(w, v)
+    too_many = torch.zeros((17, w.ny, w.nx), dtype=torch.float32, device=G.DEV)
+    out = torch.empty((w.n_probes, 17), dtype=torch.float32, device=G.DEV)
+    with pytest.raises(prism.PrismError) as e:
+        prism.compute_detectors(pp, s, beams, too_many, out, G.ws(pp, prism.WS_OUTPUT))
+    assert e.value.code == prism.PRISM_EUNSUPPORTED
