@@ -62,6 +62,11 @@ typedef struct prism_params {
                                    Results do not depend on it (PAPER.md:126 batch_size).                   */
     int32_t potential_on_host;  /* 0: V is device memory.  1: V is page-locked host memory and is streamed
                                    slice by slice over a private copy stream.            */
+    int32_t smatrix_on_host;    /* 0: S is device memory.  1: S is page-locked host memory ("the
+                                   current S-matrix subset": streaming PRISM for S-matrices beyond device memory):
+                                   prism_compute_smatrix runs `batch` beams at a time in the workspace and copies
+                                   their layers out; prism_compute_output / _patterns / _detectors copy the rows
+                                   a batch of probe rows needs into the workspace.  Regular probe lattices only. */
 } prism_params;
 
 /* Per-species radial table of the projected atomic potential ("precomputed lookup table for

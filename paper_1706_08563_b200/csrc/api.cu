@@ -411,17 +411,28 @@ static void carve_feeder(Arena& a, const prism_params* p, SliceFeeder& f, bool m
 }
 
 // ---- layouts -----------------------------------------------------------------------------------------
-struct SmatrixLayout { SliceTables tab; SliceFeeder feed; int2* beams; };
+// beams per batch of prism_compute_smatrix: all of them when S is device memory (it is the wave buffer); with S in
+// host memory the batch lives in the workspace: p->batch beams, by default about 8 GiB of waves
+static int smatrix_batch(const prism_params* p, int n_beams)
+{
+    if (p->batch > 0) return std::min<int>(p->batch, n_beams);
+    if (!p->smatrix_on_host) return n_beams;
+    const long long per_beam = (long long)p->nx * p->ny * (long long)sizeof(float2);
+    return (int)std::max<long long>(1, std::min<long long>(n_beams, (long long)(8ull << 30) / per_beam));
+}
+struct SmatrixLayout { SliceTables tab; SliceFeeder feed; int2* beams; float2* wave; };
 static void layout_smatrix(Arena& a, const prism_params* p, int n_beams, SmatrixLayout& L)
 {
     carve_slice_tables(a, p, L.tab);
-    carve_feeder(a, p, L.feed, false);          // one batch holds every beam by default
+    carve_feeder(a, p, L.feed, p->smatrix_on_host != 0 && smatrix_batch(p, n_beams) < n_beams);
     L.beams = a.take<int2>(n_beams);
+    L.wave = p->smatrix_on_host ? a.take<float2>((size_t)smatrix_batch(p, n_beams) * p->nx * p->ny) : nullptr;
 }
 
 constexpr int LATTICE_MAX_SLOTS = 4, LATTICE_MAX_Q = 32;
 struct OutputLayout {
-    float2 *tw_x, *tw_y, *coef_b, *phase_x, *phase_y, *w, *lat_coef;
+    float2 *tw_x, *tw_y, *coef_b, *phase_x, *phase_y, *w, *lat_coef, *slab;
+    int slab_rows;
     int *win_x0, *win_y0, *bin_start, *bin_pix, *cell_beam;
     float *intensity, *out_stage;
     int batch;
@@ -431,6 +442,17 @@ static void layout_output(Arena& a, const prism_params* p, int n_beams, OutputLa
     const int mx = p->nx / p->f, my = p->ny / p->f, nb = prism_num_bins(p);
     const size_t npix = (size_t)mx * my;
     L.batch = default_probe_batch(p, npix * 12);
+    L.slab = nullptr; L.slab_rows = 0;
+    if (p->smatrix_on_host) {
+        // S in host memory: a batch is whole probe rows, and the workspace holds the pixel rows of every layer that
+        // those rows' windows cover (at most ~16 GiB: fewer probe rows per batch otherwise)
+        const int sy = std::max(1, (int)std::floor(p->probe_step[1] / (p->cell[1] / p->ny) + 0.5));
+        int rows = std::min(p->probes_y, std::max(1, L.batch / std::max(1, p->probes_x)));
+        auto slab_rows = [&](int r) { return std::min(p->ny, sy * (r - 1) + my); };
+        while (rows > 1 && (size_t)n_beams * slab_rows(rows) * p->nx * sizeof(float2) > ((size_t)16 << 30)) rows /= 2;
+        L.batch = rows * p->probes_x;
+        L.slab_rows = slab_rows(rows);
+    }
     L.tw_x = a.take<float2>(mx);
     L.tw_y = a.take<float2>(my);
     L.coef_b = a.take<float2>(n_beams);
@@ -445,6 +467,7 @@ static void layout_output(Arena& a, const prism_params* p, int n_beams, OutputLa
     L.w = a.take<float2>((size_t)L.batch * npix);
     L.intensity = a.take<float>((size_t)L.batch * npix);
     L.out_stage = a.take<float>((size_t)p->probes_x * p->probes_y * nb);
+    if (p->smatrix_on_host) L.slab = a.take<float2>((size_t)n_beams * L.slab_rows * p->nx);
 }
 
 // Regular probe lattice test ("lattice DFT"): the window origins advance by a constant
@@ -787,12 +810,14 @@ int prism_compute_smatrix(const prism_params* p, const float* v, int32_t* beams_
     feed.sigma = sigma; feed.main_stream = st; feed.pairs = packed_row(p->nx, p->ny);
     if ((rc = feed.init())) { feed.release(); return rc; }
 
-    const int batch = p->batch > 0 ? std::min<int>(p->batch, n_beams) : n_beams;
+    const int batch = smatrix_batch(p, n_beams);
+    const bool s_on_host = p->smatrix_on_host != 0;
     auto run = [&]() -> int {
         for (int b0 = 0; b0 < n_beams; b0 += batch) {
             const int nb = std::min(batch, n_beams - b0);
             RowArgs ra;
-            ra.a = (float2*)s + (size_t)b0 * npix; ra.out = ra.a; ra.t = feed.tbuf;
+            // S in host memory: the batch is propagated in the workspace and its layers copied out
+            ra.a = s_on_host ? L.wave : (float2*)s + (size_t)b0 * npix; ra.out = ra.a; ra.t = feed.tbuf;
             ra.tw_x = L.tab.tw_x; ra.tw_y = L.tab.tw_y; ra.beams = L.beams + b0;
             ra.n_waves = nb; ra.nx = p->nx; ra.ny = p->ny; ra.scale = 1.f; ra.xband = xband;
             ColArgs ca;
@@ -815,6 +840,9 @@ int prism_compute_smatrix(const prism_params* p, const float* v, int32_t* beams_
             }
             ra.scale = 1.0f / (float)p->nx;
             LAUNCH(K_ROW_FINAL, launch_row_pass(ROW_FINAL, ra, st), st);
+            if (s_on_host)
+                CU(cudaMemcpyAsync((float2*)s + (size_t)b0 * npix, L.wave, (size_t)nb * npix * sizeof(float2),
+                                   cudaMemcpyDeviceToHost, st));
         }
         return PRISM_OK;
     };
@@ -913,6 +941,8 @@ static int prism_output_impl(const prism_params* p, const void* s, const int32_t
     LatticePlan lat = plan_lattice(p, beams, n_beams, wx0, wy0, mx, my);
     const int rows_per_batch = L.batch / p->probes_x;
     if (rows_per_batch < 1) lat.ok = false;
+    const bool s_on_host = p->smatrix_on_host != 0;
+    if (s_on_host && !lat.ok) return PRISM_EUNSUPPORTED;      // slabs are cut along probe rows of a regular lattice
     std::vector<float2> lcoef;
     if (lat.ok) {
         lcoef.resize(n_beams);
@@ -943,6 +973,22 @@ static int prism_output_impl(const prism_params* p, const void* s, const int32_t
             const int sy = 1 << lat.sy_log2;
             g.row0 = (int)(((long long)g.py0 * sy) % p->ny);
             g.n_pix_rows = std::min(p->ny, sy * (g.n_rows - 1) + my);
+            g.slab = 0;
+            if (s_on_host) {
+                // the job brings in the S-matrix subset it needs -- the pixel rows this batch of probe
+                // rows covers, of every layer, in one strided copy (two when the rows wrap around the cell)
+                if (g.n_pix_rows > L.slab_rows) return PRISM_ENOMEM;
+                const size_t row_bytes = (size_t)p->nx * sizeof(float2);
+                const int y_start = (wy0[0] + g.row0) % p->ny;
+                const int first = std::min(g.n_pix_rows, p->ny - y_start);
+                const size_t dpitch = (size_t)g.n_pix_rows * row_bytes, spitch = (size_t)p->ny * row_bytes;
+                CU(cudaMemcpy2DAsync(L.slab, dpitch, (const char*)s + (size_t)y_start * row_bytes, spitch,
+                                     (size_t)first * row_bytes, n_beams, cudaMemcpyHostToDevice, st));
+                if (first < g.n_pix_rows)
+                    CU(cudaMemcpy2DAsync((char*)L.slab + (size_t)first * row_bytes, dpitch, s, spitch,
+                                         (size_t)(g.n_pix_rows - first) * row_bytes, n_beams, cudaMemcpyHostToDevice, st));
+                g.s = L.slab; g.slab = 1;
+            }
             LAUNCH(K_LATTICE_DFT, launch_lattice_dft(g, st), st);
         } else {
             BeamSumArgs g;

@@ -122,8 +122,9 @@ __global__ void __launch_bounds__(256, 2) lattice_dft_kernel(LatticeArgs g)
 
     // ---- (1) G[n][m] = sum over folded beams of c'_b S_b[y][x] ----
     {
-        const size_t layer = (size_t)g.nx * g.ny;
-        const float2* src = g.s + (size_t)y * g.nx + xt + px;
+        // g.slab: g.s holds only the n_pix_rows pixel rows of this batch, row r of every layer at slab row r
+        const size_t layer = g.slab ? (size_t)g.nx * g.n_pix_rows : (size_t)g.nx * g.ny;
+        const float2* src = g.s + (size_t)(g.slab ? r : y) * g.nx + xt + px;
         float2* dst = sm + px * PS;
         if (g.n_slots == 1) {
 #pragma unroll 8

@@ -99,6 +99,7 @@ struct LatticeArgs {
     int           probes_x, probes_y;
     int           py0, n_rows;        // probe rows [py0, py0 + n_rows) of this batch
     int           row0, n_pix_rows;   // pixel rows y' = (row0 + r) mod ny, r < n_pix_rows, y' relative to y00
+    int           slab;               // 1: s is a slab [n_beams][n_pix_rows][nx] of exactly those rows (S in host memory)
 };
 cudaError_t launch_lattice_dft(const LatticeArgs& args, cudaStream_t stream);
 

@@ -34,7 +34,7 @@ class Params(C.Structure):
         ("f", C.c_int32), ("probes_x", C.c_int32), ("probes_y", C.c_int32),
         ("probe_origin", C.c_double * 2), ("probe_step", C.c_double * 2),
         ("det_step", C.c_double), ("det_max", C.c_double),
-        ("batch", C.c_int32), ("potential_on_host", C.c_int32),
+        ("batch", C.c_int32), ("potential_on_host", C.c_int32), ("smatrix_on_host", C.c_int32),
     ]
 
 
@@ -119,6 +119,7 @@ def params_from_workload(w, **override) -> Params:
     p.probe_step[:] = w.probe_step
     p.det_step, p.det_max = w.det_step, w.det_max
     p.batch, p.potential_on_host = w.batch, w.potential_on_host
+    p.smatrix_on_host = getattr(w, "smatrix_on_host", 0)
     for k, v in override.items():
         setattr(p, k, v)
     return p

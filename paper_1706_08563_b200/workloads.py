@@ -56,6 +56,7 @@ class Workload:
     det_max: float = 100.0 * MRAD
     batch: int = 0
     potential_on_host: int = 0
+    smatrix_on_host: int = 0
     n_phonons: int = 1
     jitter: float = 0.0
     config_index: int = 0
