@@ -167,16 +167,24 @@ __global__ void __launch_bounds__(ColCfg<P>::THREADS, 1) col_pipe_kernel(ColArgs
         }
         if (MODE == COL_STEP || MODE == COL_MS_INIT) fft_inverse<P>(v, tw, t, sm);
 
-        if (LOADS && k + C::NBUF < n_local) {
-            sm.sync();                               // every thread of the team is past its last exchange read
-            load(k + C::NBUF);
-        }
-
+        // Order of the tile's stores and of the refill of its buffer: with 64-byte row segments (1024-point columns)
+        // the stores go first, so that they do not queue behind the cp.async copies in the LSU (1.49 -> 1.35 ms); with
+        // wider segments the earlier prefetch wins (512 points: 0.39 ms against 0.42 ms)
+        constexpr bool STORE_FIRST = (N >= 1024);
+        auto refill = [&] {
+            if (LOADS && k + C::NBUF < n_local) {
+                sm.sync();                           // every thread of the team is past its last exchange read
+                load(k + C::NBUF);
+            }
+        };
+        if (!STORE_FIRST) refill();
         if (MODE == COL_STEP || MODE == COL_MS_INIT) {
             float2* dst = g.a + (size_t)w * N * nx + kxi;
 #pragma unroll
             for (int e = 0; e < E; ++e) dst[(size_t)(t + T * e) * nx] = v[e];
+            if (STORE_FIRST) refill();
         } else {
+            if (STORE_FIRST) refill();
             // detector-plane intensity, ky contiguous
             float* dst = g.intensity + ((size_t)w * nx + kxi) * N;
 #pragma unroll
