@@ -359,13 +359,30 @@ __global__ void __launch_bounds__(ColPkCfg<N>::THREADS, 1) col_pk_kernel(ColArgs
         if (MODE == COL_STEP || MODE == COL_MS_INIT) {
             float2 v[64];
             pk::fft_dit<P, 32>(p, v, tab, t, sm, sync);
-            if (LOADS && k + C::NBUF < n_local) {
-                sync();                              // every thread of the team is past its last exchange read
-                load(k + C::NBUF);
-            }
             float2* dst = g.a + (size_t)w * N * nx + kxi;
+            if (LOADS && k + C::NBUF < n_local) {
+                // refill copies and tile stores interleaved (two stores, one 16-byte copy), so that neither kind
+                // queues up alone in the LSU
+                sync();                              // every thread of the team is past its last exchange read
+                int w2, kx2;
+                locate(k + C::NBUF, w2, kx2);
+                const float2* src = g.a + (size_t)w2 * N * nx + kx2;
+                float2* nbuf = reinterpret_cast<float2*>(bufs + (size_t)((k + C::NBUF) % C::NBUF) * C::BUF_BYTES);
+                constexpr int CH = W / 2;
+                static_assert(N * CH / C::TEAM == 32, "interleave ratio");
 #pragma unroll
-            for (int e = 0; e < 64; ++e) dst[(size_t)(t + T * e) * nx] = make_float2(v[e].y, v[e].x);
+                for (int i = 0; i < 32; ++i) {
+                    dst[(size_t)(t + T * (2 * i)) * nx] = make_float2(v[2 * i].y, v[2 * i].x);
+                    dst[(size_t)(t + T * (2 * i + 1)) * nx] = make_float2(v[2 * i + 1].y, v[2 * i + 1].x);
+                    const int q = tt + i * C::TEAM;
+                    const int row = q / CH, cc = q % CH;
+                    cp_async16(nbuf + row * W + 2 * cc, src + (size_t)row * nx + 2 * cc);
+                }
+                cp_async_arrive(&full[(k + C::NBUF) % C::NBUF]);
+            } else {
+#pragma unroll
+                for (int e = 0; e < 64; ++e) dst[(size_t)(t + T * e) * nx] = make_float2(v[e].y, v[e].x);
+            }
         } else {
             if (k + C::NBUF < n_local) {
                 sync();
