@@ -127,7 +127,7 @@ __global__ void __launch_bounds__(256, 2) lattice_dft_kernel(LatticeArgs g)
         const float2* src = g.s + (size_t)(g.slab ? r : y) * g.nx + xt + px;
         float2* dst = sm + px * PS;
         if (g.n_slots == 1) {
-#pragma unroll 8
+#pragma unroll 16
             for (int c = c0; c < Q * Q; c += CPI) {
                 const int b = __ldg(g.cell_beam + c);
                 float2 r = make_float2(0.f, 0.f);           // residues no beam folds onto: no load
