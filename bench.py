@@ -2,11 +2,16 @@
 """bench.py -- one JSON line for the PRISM hot path on N B200s (contract: task prompt / DESIGN.md).
 
 A step = one pass of the whole hot path for one frozen-phonon configuration of the workload:
-prism_build_potential -> prism_compute_smatrix -> prism_compute_output (all section 8(a) rows).
-`value` = PRISM probes/s over the whole job (all ranks), device-timed with CUDA events on the
-launching stream; `beam_slices_per_s` is reported beside it (BASELINE.json names both).
+prism_build_potential -> prism_compute_smatrix -> prism_compute_output -> prism_accumulate (all section
+8(a) rows).  `value` = PRISM probes/s over the whole job (all ranks), device-timed with CUDA events on the
+launching stream with the library's per-kernel timing OFF; `beam_slices_per_s` is reported beside it
+(BASELINE.json names both).  Per-kernel times and the roofline come from a separate, instrumented pass.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload P8|P4|P16|PR1] [--impl reference]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload P16|P8|P4|PR1|MS2] [--impl reference]
+
+The default workload is BASELINE.json configs[4] (P16: 2048^2, 400 slices streamed from pinned host memory,
+1201 beams, 512^2 probes), the largest single-GPU configuration; at N = 1 the line also carries short runs of
+the other configurations under "other_workloads" (--no-others skips them).
 
 N > 1 (torchrun): frozen-phonon configurations are independent problems, so rank r
 takes configurations r, r+N, ... with no collective on the data path ("weak" scaling); the only
@@ -15,6 +20,7 @@ exchange is one NCCL all-reduce of the [probes][rings] sums for the phonon avera
 from __future__ import annotations
 
 import argparse
+import glob
 import json
 import os
 import statistics
@@ -48,15 +54,14 @@ def measured_peaks():
 
 def measured_traffic(workload: str, kernel: str):
     """DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of one `ncu --set full` capture of this
-    kernel on this workload, from profiles/r01_traffic.csv (the .md beside it names the commands); None if absent."""
-    path = os.path.join(ROOT, "profiles", "r01_traffic.csv")
-    if not os.path.exists(path):
-        return None
-    with open(path) as fh:
-        for line in fh:
-            f = [x.strip() for x in line.split(",")]
-            if len(f) >= 3 and f[0] == workload and f[1] == kernel:
-                return float(f[2])
+    kernel on this workload, from the newest profiles/rNN_traffic.csv that lists it (the .md beside each names the
+    commands); None if absent."""
+    for path in sorted(glob.glob(os.path.join(ROOT, "profiles", "r*_traffic.csv")), reverse=True):
+        with open(path) as fh:
+            for line in fh:
+                f = [x.strip() for x in line.split(",")]
+                if len(f) >= 3 and f[0] == workload and f[1] == kernel:
+                    return float(f[2])
     return None
 
 
@@ -105,44 +110,53 @@ def oracle_params(O, w):
                     w.defocus, w.cs, w.f, w.det_step, w.det_max)
 
 
-def oracle_sample(w, budget_s: float = 20.0):
-    """Time the oracle, as it stands, on a bounded sample of the workload and extrapolate linearly in
-    beams and probes (the paper's own practice).  Returns (probes/s, description, dict)."""
+def oracle_sample(w, budget_s: float = 25.0):
+    """Time the oracle, as it stands (unoptimised fp64 C with its own radix-2 FFT), on a bounded sample of the
+    workload: whole beams (one per host thread) through the first min(S, 50) slices -- fewer only when 50 slices
+    would exceed the time budget -- and 2 probes per thread on a reduced beam set; anything not run in full is
+    scaled linearly in beams, slices and probes (the paper's own practice) and the result is
+    marked `extrapolated`.  Returns (probes/s, description, cores, detail)."""
     import oracle as O
-    from paper_1706_08563_b200 import workloads  # noqa: F401  (inputs only)
     cores = O.num_threads()
     p = oracle_params(O, w)
     lut_z, r_cut, lut_v = w.lut()
     atoms = w.atoms_for_phonon(0)
     beams = O.beams(p)
     n_beams, n_probes = len(beams), w.n_probes
-    # potential: full size is affordable only for small grids; sample a slab of slices otherwise
-    s_slab = w.n_slices if w.nx <= 256 else max(1, min(w.n_slices, 2))
+    nb = min(n_beams, cores)
+    # calibrate on one slice, then take as many slices as the budget allows, at most 50
+    p1 = oracle_params(O, w.with_(n_slices=1))
+    sel1 = atoms[:, 2] < w.dz
+    v1 = O.potential(p1, atoms[sel1], w.z[sel1], lut_z, r_cut, lut_v)
+    t0 = time.perf_counter()
+    O.smatrix(p1, v1, beams[:nb])
+    t_one = time.perf_counter() - t0
+    s_slab = int(max(1, min(w.n_slices, 50, budget_s // max(t_one, 1e-3))))
     p_slab = oracle_params(O, w.with_(n_slices=s_slab))
     sel = atoms[:, 2] < s_slab * w.dz
     t0 = time.perf_counter()
     v = O.potential(p_slab, atoms[sel], w.z[sel], lut_z, r_cut, lut_v)
     t_pot = (time.perf_counter() - t0) * (w.n_slices / s_slab)
-    # stage 1: `cores` beams through the slab, one per thread
-    nb = min(n_beams, cores)
+    # stage 1: nb whole beams through the slab, one per thread
     t0 = time.perf_counter()
     O.smatrix(p_slab, v, beams[:nb])
-    t_bs = (time.perf_counter() - t0) / (nb * s_slab) * cores          # core-seconds per beam-slice
+    t_bs = (time.perf_counter() - t0) * min(nb, cores) / (nb * s_slab)      # core-seconds per beam-slice
     t_s1 = t_bs * n_beams * w.n_slices / cores
-    # stage 2: `cores` probes on a reduced beam set (cost is linear in beams), seeded random S-matrix
+    # stage 2: 2 probes per thread on a reduced beam set (cost is linear in beams), seeded random S-matrix
     nb2 = min(n_beams, max(4, int(2.0e9 // (w.nx * w.ny * 16))))
     rng = np.random.default_rng(1)
     s = (rng.standard_normal((nb2, w.ny, w.nx)) + 1j * rng.standard_normal((nb2, w.ny, w.nx)))
     npr = min(n_probes, cores * 2)
     t0 = time.perf_counter()
     O.prism_probes(p, s, beams[:nb2], w.probe_xy()[:npr])
-    t_pr = (time.perf_counter() - t0) / npr * cores                    # core-seconds per probe at nb2 beams
+    t_pr = (time.perf_counter() - t0) * min(npr, cores) / npr                # core-seconds per probe at nb2 beams
     t_s2 = t_pr * (n_beams / nb2) * n_probes / cores
     total = t_pot + t_s1 + t_s2
-    desc = (f"oracle (fp64 C, gcc -O2, OpenMP x{cores}) on a sample of {w.name}: potential {s_slab}/{w.n_slices} "
-            f"slices, {nb} beams x {s_slab} slices, {npr} probes x {nb2}/{n_beams} beams; scaled linearly to "
-            f"{n_beams} beams x {w.n_slices} slices and {n_probes} probes")
-    detail = {"potential_s": t_pot, "smatrix_s": t_s1, "output_s": t_s2,
+    extrapolated = s_slab < w.n_slices or nb < n_beams or nb2 < n_beams or npr < n_probes
+    desc = (f"unoptimised fp64 oracle (plain C, own radix-2 FFT, gcc -O2, OpenMP x{cores}) on a sample of {w.name}: "
+            f"potential {s_slab}/{w.n_slices} slices, {nb} whole beams x {s_slab} slices, {npr} probes x "
+            f"{nb2}/{n_beams} beams; scaled linearly to {n_beams} beams x {w.n_slices} slices and {n_probes} probes")
+    detail = {"potential_s": t_pot, "smatrix_s": t_s1, "output_s": t_s2, "extrapolated": bool(extrapolated),
               "beam_slices_per_s": n_beams * w.n_slices / t_s1}
     return n_probes / total, desc, cores, detail
 
@@ -165,21 +179,24 @@ def run_reference_multislice(args, w):
         if i >= args.warmup:
             vals.append(w.n_probes / (t_pot + dt * w.n_probes / len(xy)))
     value = float(np.mean(vals))
-    desc = (f"oracle (fp64 C, gcc -O2, OpenMP x{cores}): whole potential, {len(xy)} of {w.n_probes} probes through "
-            f"{w.n_slices} slices, scaled linearly in probes")
+    desc = (f"unoptimised fp64 oracle (plain C, gcc -O2, OpenMP x{cores}): whole potential, {len(xy)} of {w.n_probes} "
+            f"probes through {w.n_slices} slices, scaled linearly in probes")
     print(json.dumps({
         "impl": "reference", "metric": "multislice_probes_per_s", "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": len(vals), "warmup": args.warmup, "ms_per_step": 1e3 * w.n_probes / value, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": f"{w.name} ({WORKLOAD_NOTE.get(w.name, 'test case')}): plain multislice, {w.nx}x{w.ny}, "
                                f"{w.n_slices} slices, {w.probes_x}x{w.probes_y} probes"},
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc,
+                         "extrapolated": True},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
 
 
 def run_reference(args):
     """--impl reference: the oracle is the reference arm for this tier (no pip-installable reference exists:
-    /root/reference holds only the paper text)."""
+    /root/reference holds only the paper text).  Each step is one bounded sample of the workload, scaled
+    linearly (`cpu_baseline.extrapolated`), so `ms_per_step` is the extrapolated time of a whole step, not the
+    wall time of the sample."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
@@ -191,12 +208,12 @@ def run_reference(args):
     t_begin = time.perf_counter()
     for i in range(args.warmup + args.steps):
         # each step is one bounded sample; keep the whole run within a few minutes
-        budget_left = 240.0 - (time.perf_counter() - t_begin)
+        budget_left = 200.0 - (time.perf_counter() - t_begin)
         if i >= 1 and budget_left < 0 and vals:
             break
-        val, desc, cores, detail = oracle_sample(w)
+        val, desc, cores, detail = oracle_sample(w, budget_s=12.0)
         last = (desc, cores, detail)
-        if i >= args.warmup or i == args.warmup + args.steps - 1:
+        if i >= args.warmup or i == args.warmup + args.steps - 1 or budget_left < 60.0:
             vals.append(val)
     value = float(np.mean(vals))
     desc, cores, detail = last
@@ -204,15 +221,17 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": len(vals), "warmup": args.warmup, "ms_per_step": 1e3 * w.n_probes / value,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": workload_config(w, args),
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+        "config": workload_config(w),
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc,
+                         "extrapolated": detail["extrapolated"]},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "beam_slices_per_s": detail["beam_slices_per_s"],
+        "note": "ms_per_step is extrapolated from the bounded sample (steps x ms_per_step is not the wall time of this run)",
     }
     print(json.dumps(line))
 
 
-def workload_config(w, args):
+def workload_config(w):
     return {"workload": f"{w.name} ({WORKLOAD_NOTE.get(w.name, 'test case')}): {w.nx}x{w.ny} grid, "
                         f"{w.n_slices} slices, f={w.f}, {w.probes_x}x{w.probes_y} probes, "
                         f"{len(w.z)} atoms, one frozen-phonon configuration per step",
@@ -222,21 +241,16 @@ def workload_config(w, args):
                   if w.nx >= 512 else "working set fits L2; L2 flushed between steps by the workspace writes"}
 
 
-
 # ------------------------------------------------------------------------------------------------ multislice line
-def run_multislice(args):
-    """--workload MS2 (BASELINE.json configs[1], the comparison path): a step is prism_build_potential ->
+def run_multislice(args, name, steps, warmup):
+    """Workload MS2 (BASELINE.json configs[1], the comparison path): a step is prism_build_potential ->
     multislice_compute_output over the whole probe grid in the configuration's batches of 64 probes.  Reported as
-    multislice probes/s; one GPU only (the default PRISM line is the one the driver reads)."""
+    multislice probes/s; one GPU only."""
     import torch
     from paper_1706_08563_b200 import prism, workloads
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
-    if int(os.environ.get("RANK", "0")) != 0:
-        return
     dev = torch.device("cuda", int(os.environ.get("LOCAL_RANK", "0")))
     torch.cuda.set_device(dev)
-    w = workloads.get(args.workload)
+    w = workloads.get(name)
     p = prism.params_from_workload(w)
     lut_z, r_cut, lut_v = w.lut()
     atoms = np.ascontiguousarray(w.atoms_for_phonon(0))
@@ -251,7 +265,7 @@ def run_multislice(args):
         prism.build_potential(p, atoms, w.z, lut_z, r_cut, lut_v, v, ws)
         prism.multislice_output(p, v, target, ws)
 
-    for _ in range(args.warmup):
+    for _ in range(warmup):
         step(out_dev)
     torch.cuda.synchronize()
     sampler = ClockSampler(dev.index or 0)
@@ -259,23 +273,23 @@ def run_multislice(args):
     prism.launch_count(reset=True)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record()
-    for _ in range(args.steps):
+    for _ in range(steps):
         step(out_dev)
     e1.record()
     torch.cuda.synchronize()
-    ms_per_step = e0.elapsed_time(e1) / args.steps
+    ms_per_step = e0.elapsed_time(e1) / steps
     launches = prism.launch_count()
-    # per-kernel times come from a second, instrumented pass: this path is launch-bound (1700 launches of ~15 us per
-    # step) and a pair of events around every launch would slow the timed region itself by a quarter
+    clocks = sampler.stop()
+    # per-kernel times come from a second, instrumented pass (a pair of events around every launch would slow
+    # the timed region itself)
     prism.timing_enable(True)
-    for _ in range(args.steps):
+    for _ in range(steps):
         step(out_dev)
     torch.cuda.synchronize()
     prism.timing_enable(False)
     kern = prism.timing_read()
-    clocks = sampler.stop()
     t0 = time.perf_counter()
-    for _ in range(args.steps):
+    for _ in range(steps):
         step(out_host)
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
@@ -284,64 +298,40 @@ def run_multislice(args):
     band = 2.0 * prism.band_columns(p) / w.nx if min(w.nx, w.ny) >= 256 else 1.0
     per_launch = 16.0 * npix * band * min(batch, n_probes)              # one pass over one batch of probes
     kernels = {}
-    for name, (ms, cnt) in kern.items():
-        entry = {"ms_per_step": ms / args.steps, "launches_per_step": cnt / args.steps, "avg_ms": ms / cnt}
-        if name in ("row_step", "col_step"):
+    for kname, (ms, cnt) in kern.items():
+        entry = {"ms_per_step": ms / steps, "launches_per_step": cnt / steps, "avg_ms": ms / cnt}
+        if kname in ("row_step", "col_step"):
             entry["algorithmic_GBps"] = per_launch / (ms / cnt * 1e-3) / 1e9
-        kernels[name] = entry
+        kernels[kname] = entry
     top = max(kernels, key=lambda n: kernels[n]["ms_per_step"])
     ach = kernels[top].get("algorithmic_GBps", 0.0)
-    line = {
+    return {
         "metric": "multislice_probes_per_s", "value": n_probes / (ms_per_step * 1e-3), "unit": UNIT, "n_gpus": 1,
-        "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True,
+        "steps": steps, "warmup": warmup, "ms_per_step": ms_per_step, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "complex64", "data": "synthetic",
         "config": {"workload": f"{w.name} ({WORKLOAD_NOTE.get(w.name, 'test case')}): {w.nx}x{w.ny} grid, {w.n_slices} slices, "
                                f"{w.probes_x}x{w.probes_y} probes in batches of {batch}, {len(w.z)} atoms, plain multislice",
                    "l2": "a batch of 64 waves (33.5 MB) fits L2; the three-batch rotation of the timed loop does not flush it"},
         "clocks": clocks,
-        "e2e": {"value": n_probes * args.steps / e2e_s, "unit": UNIT,
+        "e2e": {"value": n_probes * steps / e2e_s, "unit": UNIT,
                 "h2d_bytes_per_step": int(24 * len(w.z) + lut_v.size * 4 + 8 * (w.probes_x * w.nx + w.probes_y * w.ny + npix)),
                 "d2h_bytes_per_step": int(out_host.numel() * 4)},
-        "gpu_launches": int(launches),
+        "gpu_launches": int(launches), "launches_per_step": launches / steps,
         "roofline": {"kernel": top, "bound": "hbm", "achieved": ach, "peak": hbm_peak, "unit": "GB/s",
                      "frac": ach / hbm_peak, "traffic": None, "peak_source": peak_src, "bytes_per_launch": per_launch,
                      "note": "launch-sized batches: the waves of a batch stay in L2, so this is not an HBM measurement"},
         "kernels": kernels,
     }
-    print(json.dumps(line))
+
 
 # ------------------------------------------------------------------------------------------------ CUDA arm
-def main():
-    ap = argparse.ArgumentParser()
-    ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=5)
-    ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="P8", choices=["PR1", "MS2", "P4", "P8", "P16"])
-    ap.add_argument("--no-cpu-baseline", action="store_true")
-    args = ap.parse_args()
-    if args.impl == "reference":
-        return run_reference(args)
-    if args.workload == "MS2":
-        return run_multislice(args)
-
+def run_prism(name, steps, warmup, world, rank, local, dist, want_cpu_baseline):
+    """The PRISM line of one workload.  Returns the JSON-able dict (on every rank; rank 0 prints it)."""
     import torch
     from paper_1706_08563_b200 import prism, sharding, workloads
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
-    torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
-    dist = None
-    if world > 1:
-        import torch.distributed as dist_mod
-        dist = dist_mod
-        dist.init_process_group("nccl", device_id=dev)
-
-    w = workloads.get(args.workload)
+    w = workloads.get(name)
     p = prism.params_from_workload(w)
     lut_z, r_cut, lut_v = w.lut()
     n_beams, n_bins, n_probes = prism.num_beams(p), prism.num_bins(p), w.n_probes
@@ -354,46 +344,40 @@ def main():
     s = torch.empty((n_beams, w.ny, w.nx), dtype=torch.complex64, device=dev)
     out_dev = torch.empty((w.probes_y, w.probes_x, n_bins), dtype=torch.float32, device=dev)
     out_host = torch.empty((w.probes_y, w.probes_x, n_bins), dtype=torch.float32).pin_memory()
-    acc = torch.zeros_like(out_dev)
+    acc = torch.empty_like(out_dev)
     ws_bytes = max(prism.workspace_bytes(p, prism.WS_POTENTIAL, len(w.z)), prism.workspace_bytes(p, prism.WS_SMATRIX),
                    prism.workspace_bytes(p, prism.WS_OUTPUT))
     ws = torch.empty(ws_bytes, dtype=torch.uint8, device=dev)
-    # comparison path: plain multislice on a coarse sub-grid of the probe positions
-    ms_n = max(1, min(8, w.probes_x, w.probes_y))
-    w_ms = w.with_(probes_x=ms_n, probes_y=ms_n, probe_step=(w.cell[0] / ms_n, w.cell[1] / ms_n))
-    p_ms = prism.params_from_workload(w_ms)
-    out_ms = torch.empty((ms_n, ms_n, n_bins), dtype=torch.float32, device=dev)
-    ws_ms = torch.empty(prism.workspace_bytes(p_ms, prism.WS_MULTISLICE), dtype=torch.uint8, device=dev)
     # frozen-phonon configurations of this rank (host inputs, prepared outside the timed region)
     my_phonons = sharding.phonons_for_rank(w.n_phonons, world, rank)
     atoms = {ph: np.ascontiguousarray(w.atoms_for_phonon(ph)) for ph in my_phonons}
-    beams_holder = {}
 
     def step(k, out_target):
         ph = my_phonons[k % len(my_phonons)]
         prism.build_potential(p, atoms[ph], w.z, lut_z, r_cut, lut_v, v, ws)
-        beams_holder["b"] = prism.compute_smatrix(p, v, s, ws)
-        prism.compute_output(p, s, beams_holder["b"], out_target, ws)
+        beams = prism.compute_smatrix(p, v, s, ws)
+        prism.compute_output(p, s, beams, out_target, ws)
+        return beams
 
     def barrier():
         if dist is not None:
             dist.barrier()
         torch.cuda.synchronize()
 
-    for k in range(args.warmup):
+    for k in range(warmup):
         step(k, out_dev)
     barrier()
 
-    # ---- timed region: device-resident output, CUDA events on the launching stream ----
+    # ---- timed region: device-resident output, CUDA events on the launching stream, library timing OFF ----
     sampler = ClockSampler(local)
     sampler.start()
     prism.launch_count(reset=True)
-    prism.timing_enable(True)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    stage_ev = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(args.steps)]
+    stage_ev = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(steps)]
+    weight = 1.0 / (steps * world)
     barrier()
     e0.record()
-    for k in range(args.steps):
+    for k in range(steps):
         ph = my_phonons[k % len(my_phonons)]
         stage_ev[k][0].record()
         prism.build_potential(p, atoms[ph], w.z, lut_z, r_cut, lut_v, v, ws)
@@ -402,28 +386,36 @@ def main():
         stage_ev[k][2].record()
         prism.compute_output(p, s, beams, out_dev, ws)
         stage_ev[k][3].record()
-        acc += out_dev
-    sharding.phonon_average(acc, args.steps, dist)                # frozen-phonon average
+        prism.accumulate(acc, out_dev, weight, first=(k == 0))          # frozen-phonon average
+    sharding.all_reduce_sum(acc, dist)
     e1.record()
     barrier()
     ms_total = e0.elapsed_time(e1)
     launches = prism.launch_count()
-    prism.timing_enable(False)
-    kern = prism.timing_read()
     clocks = sampler.stop()
-    stage_ms = [float(np.mean([stage_ev[k][i].elapsed_time(stage_ev[k][i + 1]) for k in range(args.steps)]))
+    stage_ms = [float(np.mean([stage_ev[k][i].elapsed_time(stage_ev[k][i + 1]) for k in range(steps)]))
                 for i in range(3)]
     if dist is not None:
         t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         ms_total = float(t.item())
-    ms_per_step = ms_total / args.steps
+    ms_per_step = ms_total / steps
     value = world * n_probes / (ms_per_step * 1e-3)
 
-    # ---- end to end: same calls, result delivered into pinned HOST memory inside the timed region ----
+    # ---- instrumented pass: the same step with a pair of events around every launch (per-kernel table, roofline) ----
+    inst_steps = max(1, min(steps, 3 if ms_per_step < 2000.0 else 1))
+    prism.timing_enable(True)
+    for k in range(inst_steps):
+        step(k, out_dev)
+    torch.cuda.synchronize()
+    prism.timing_enable(False)
+    kern = prism.timing_read()
+
+    # ---- end to end: same calls, host atoms in, result delivered into pinned HOST memory inside the timed region ----
+    e2e_steps = max(1, min(steps, max(3, int(90e3 / ms_per_step))))
     barrier()
     t0 = time.perf_counter()
-    for k in range(args.steps):
+    for k in range(e2e_steps):
         step(k, out_host)
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
@@ -431,8 +423,19 @@ def main():
         t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         e2e_s = float(t.item())
-    # ---- comparison path: multislice probes/s on ms_n x ms_n probes through the same slice-step kernels ----
-    prism.multislice_output(p_ms, v, out_ms, ws_ms)                  # warm-up
+    # ---- comparison path: plain multislice through the same slice-step kernels ----
+    # P16: BASELINE.json configs[4] names the run (64 x 64 probes on the same grid and slices); elsewhere a coarse
+    # 8 x 8 sub-grid of the probe positions
+    ms_n = 64 if name == "P16" else max(1, min(8, w.probes_x, w.probes_y))
+    w_ms = w.with_(probes_x=ms_n, probes_y=ms_n, probe_step=(w.cell[0] / ms_n, w.cell[1] / ms_n),
+                   batch=256 if name == "P16" else w.batch)
+    p_ms = prism.params_from_workload(w_ms)
+    del ws
+    torch.cuda.empty_cache()
+    out_ms = torch.empty((ms_n, ms_n, n_bins), dtype=torch.float32, device=dev)
+    ws_ms = torch.empty(prism.workspace_bytes(p_ms, prism.WS_MULTISLICE), dtype=torch.uint8, device=dev)
+    if name != "P16":
+        prism.multislice_output(p_ms, v, out_ms, ws_ms)                  # warm-up (the P16 run is long enough without)
     barrier()
     m0, m1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     m0.record()
@@ -440,18 +443,15 @@ def main():
     m1.record()
     barrier()
     ms_probes_per_s = world * ms_n * ms_n / (m0.elapsed_time(m1) * 1e-3)
-    del ws_ms
+    ms_sweeps = -(-ms_n * ms_n // (w_ms.batch if w_ms.batch > 0 else ms_n * ms_n))
+    del ws_ms, out_ms, s
+    torch.cuda.empty_cache()
     cells = w.n_slices * (w.nx // 16) * (w.ny // 16)
     v_bytes = 4 * npix * w.n_slices if w.potential_on_host else 0
     h2d = 24 * len(w.z) + 4 * (cells + 1) + lut_v.size * 4 + v_bytes + 8 * (2 * w.nx + 2 * w.ny) \
         + 8 * n_beams * (w.probes_x + w.probes_y + 2) + 4 * (w.nx // w.f) * (w.ny // w.f)
     d2h = out_host.numel() * 4 + v_bytes
-    e2e_value = world * n_probes * args.steps / e2e_s
-
-    if rank != 0:
-        if dist is not None:
-            dist.destroy_process_group()
-        return
+    e2e_value = world * n_probes * e2e_steps / e2e_s
 
     # ---- roofline of the dominant kernel (16 N^2 bytes per wave and pass; 8 N_b M^2 flop per probe) --
     hbm_peak, peak_src = measured_peaks()
@@ -462,13 +462,14 @@ def main():
     mixed, real = 8 * npix * n_beams * band, 8 * npix * n_beams
     per_launch_bytes = {"row_step": 2 * mixed, "col_step": 2 * mixed, "row_init": mixed, "row_final": mixed + real}
     kernels = {}
-    for name, (ms, cnt) in kern.items():
-        entry = {"ms_per_step": ms / args.steps, "launches_per_step": cnt / args.steps, "avg_ms": ms / cnt}
-        if name in per_launch_bytes:
-            entry["algorithmic_GBps"] = per_launch_bytes[name] / (ms / cnt * 1e-3) / 1e9
-        if name == "beam_sum":
-            entry["algorithmic_TFLOPs"] = 8.0 * n_beams * m2 * n_probes * args.steps / (ms * 1e-3) / 1e12
-        kernels[name] = entry
+    for kname, (ms, cnt) in kern.items():
+        entry = {"ms_per_step": ms / inst_steps, "launches_per_step": cnt / inst_steps, "avg_ms": ms / cnt}
+        if kname in per_launch_bytes:
+            entry["algorithmic_GBps"] = per_launch_bytes[kname] / (ms / cnt * 1e-3) / 1e9
+            entry["frac_of_hbm_peak"] = entry["algorithmic_GBps"] / hbm_peak
+        if kname == "beam_sum":
+            entry["algorithmic_TFLOPs"] = 8.0 * n_beams * m2 * n_probes * inst_steps / (ms * 1e-3) / 1e12
+        kernels[kname] = entry
     top = max(kernels, key=lambda n: kernels[n]["ms_per_step"])
     if top in per_launch_bytes:
         ach = kernels[top]["algorithmic_GBps"]
@@ -489,27 +490,91 @@ def main():
                               "unbanded_32N2_GBps": 32.0 * npix * n_beams * w.n_slices / (slice_ms * 1e-3) / 1e9,
                               "fp32_TFLOPs_nominal": flops / (slice_ms * 1e-3) / 1e12,
                               "fp32_frac": flops / (slice_ms * 1e-3) / 1e12 / FP32_PEAK_TFLOPS}
+    roofline["measured_in"] = (f"instrumented pass of {inst_steps} step(s) after the timed region (CUDA events around "
+                               "every launch on the launching stream)")
 
     line = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": warmup,
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "complex64", "data": "synthetic", "config": workload_config(w, args), "clocks": clocks,
-        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h)},
-        "gpu_launches": int(launches),
+        "dtype": "complex64", "data": "synthetic", "config": workload_config(w), "clocks": clocks,
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+                "steps": e2e_steps},
+        "gpu_launches": int(launches), "launches_per_step": launches / steps,
         "beam_slices_per_s": world * n_beams * w.n_slices / (stage_ms[1] * 1e-3),
         "stage2_probes_per_s": world * n_probes / (stage_ms[2] * 1e-3),
         "stage_ms": {"potential": stage_ms[0], "smatrix": stage_ms[1], "output": stage_ms[2]},
         "multislice": {"probes_per_s": ms_probes_per_s, "probes": ms_n * ms_n,
+                       "potential_sweeps": ms_sweeps,
+                       "h2d_bytes": int(ms_sweeps * v_bytes),
                        "note": "comparison path (row M1): same potential and slice-step kernels, one probe per wave; "
                                "PRISM / multislice speed-up = stage2_probes_per_s / probes_per_s once the S-matrix is built",
                        "prism_over_multislice": (world * n_probes / (ms_per_step * 1e-3)) / ms_probes_per_s},
         "roofline": roofline, "kernels": kernels,
     }
-    if world == 1 and not args.no_cpu_baseline:
+    if want_cpu_baseline and rank == 0:
         val, desc, cores, detail = oracle_sample(w)
         line["cpu_baseline"] = {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc,
+                                "extrapolated": detail["extrapolated"],
                                 "beam_slices_per_s": detail["beam_slices_per_s"]}
-    print(json.dumps(line))
+    return line
+
+
+def compact(line):
+    """The keys of a full line that matter when it is reported under "other_workloads"."""
+    keep = ("metric", "value", "unit", "steps", "warmup", "ms_per_step", "config", "e2e", "launches_per_step",
+            "beam_slices_per_s", "stage2_probes_per_s", "stage_ms", "roofline")
+    out = {k: line[k] for k in keep if k in line}
+    out["config"] = {"workload": line["config"]["workload"]}
+    if "kernels" in line:
+        out["kernels"] = {k: {kk: vv for kk, vv in e.items() if kk in ("avg_ms", "algorithmic_GBps", "frac_of_hbm_peak")}
+                          for k, e in line["kernels"].items()}
+    return out
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="P16", choices=["PR1", "MS2", "P4", "P8", "P16"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-others", action="store_true",
+                    help="skip the short runs of the other configurations reported under other_workloads")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+
+    if args.workload == "MS2":
+        if rank == 0:
+            print(json.dumps(run_multislice(args, "MS2", args.steps, args.warmup)))
+        return
+
+    dist = None
+    if world > 1:
+        import torch.distributed as dist_mod
+        dist = dist_mod
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    line = run_prism(args.workload, args.steps, args.warmup, world, rank, local, dist,
+                     want_cpu_baseline=(world == 1 and not args.no_cpu_baseline))
+    if rank == 0 and world == 1 and args.workload == "P16" and not args.no_others:
+        # the other BASELINE.json configurations, short runs on the same box (context; the line above is the headline)
+        others = {}
+        for other in ("P8", "P4"):
+            others[other] = compact(run_prism(other, 5, 3, 1, 0, local, None, want_cpu_baseline=False))
+        others["MS2"] = compact(run_multislice(args, "MS2", 5, 3))
+        line["other_workloads"] = others
+    if rank == 0:
+        print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()
 

@@ -11,12 +11,21 @@
  * 1/N; array slot m holds signed frequency k = m (m < N/2) or m - N.
  *
  * Ownership: the caller owns every buffer (V, S, out, workspace) and the CUDA
- * stream.  The library allocates no device memory, keeps no state between calls
- * ("perform all memory allocations initially"), and enqueues its work
- * on the given stream; outputs are valid once the caller has synchronised that
- * stream.  Host-side tables are built in fp64 inside each call.  When a potential
- * is streamed from host memory the library uses a private copy stream and events,
- * created and released inside the call; all of its copies are joined into `stream`.
+ * stream.  The library allocates no device memory ("perform all memory
+ * allocations initially") and keeps no simulation state between calls: every call is
+ * a function of its arguments.  What it does keep, process-wide, is bookkeeping:
+ * per-device marks for one-time kernel set-up (shared-memory opt-in, occupancy), a
+ * launch counter, and -- only while prism_timing_enable is on -- a list of timing
+ * events.  Calls may be made concurrently from several host threads (one per device
+ * or stream, the paper's multi-GPU model); the bookkeeping is atomic or
+ * mutex-guarded.
+ * Work is enqueued on the given stream; outputs are valid once the caller has
+ * synchronised that stream.  Host-side tables are built in fp64 inside each call and
+ * uploaded from call-local host memory, so each compute call blocks the calling host
+ * thread once, until its own table uploads have been consumed (they queue behind work
+ * already on the stream); the kernels then run asynchronously.  When a potential is
+ * streamed from host memory the library uses a private copy stream and events, created
+ * and released inside the call; all of its copies are joined into `stream`.
  *
  * Errors: every int-returning function returns PRISM_OK (0) or a negative code;
  * nothing aborts, nothing throws across the ABI.  There is no CPU fallback: on a
@@ -157,6 +166,12 @@ int prism_compute_detectors(const prism_params* p, const void* s, const int32_t*
 int multislice_compute_detectors(const prism_params* p, const float* v, const float* masks, int32_t n_masks,
                                  float* out, void* workspace, size_t workspace_bytes, void* cuda_stream);
 
+/* Frozen-phonon average ("32 frozen phonon configurations" are averaged): the caller loops over
+ * configurations -- each one a full run of the calls above on freshly displaced atoms -- and accumulates
+ *   acc[i] = (first ? 0 : acc[i]) + weight * x[i],  i < n      (weight = 1 / n_configurations gives the mean).
+ *   acc, x  DEVICE fp32 [n] (any output of the calls above: rings, patterns, detectors). */
+int prism_accumulate(float* acc, const float* x, int64_t n, float weight, int32_t first, void* cuda_stream);
+
 /* Text for an error code, and the message of the last CUDA failure seen by the calling thread. */
 const char* prism_strerror(int code);
 const char* prism_last_error(void);
@@ -166,7 +181,9 @@ int64_t prism_launch_count(int32_t reset);
 /* Optional device timing per kernel class (measurement aid): when enabled, every
  * launch is bracketed by a pair of CUDA events on the stream it is launched on.  prism_timing_read()
  * waits for the recorded launches, adds their durations (ms) and counts per class into the two arrays
- * (prism_timing_classes() entries each) and clears the record.  Not thread-safe; off by default. */
+ * (prism_timing_classes() entries each) and clears the record.  The record is process-wide (all threads and
+ * streams together, mutex-guarded); off by default.  While it is on, the event between two launches keeps the
+ * next kernel's prologue from overlapping the previous kernel, so timed runs are slightly slower. */
 int32_t     prism_timing_enable(int32_t enable);          /* returns the previous setting */
 int32_t     prism_timing_classes(void);
 const char* prism_timing_class_name(int32_t cls);

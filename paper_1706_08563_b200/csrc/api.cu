@@ -9,6 +9,7 @@
 #include <cstdio>
 #include <cstring>
 #include <memory>
+#include <mutex>
 #include <vector>
 
 #include "../../include/prism.h"
@@ -34,32 +35,41 @@ static int cuda_fail(cudaError_t e, const char* what)
 // CUDA events around every launch, on the stream the kernel is launched on.
 enum KernelClass { K_POTENTIAL = 0, K_TRANSMISSION, K_ROW_INIT, K_ROW_STEP, K_ROW_FINAL, K_COL_STEP,
                    K_BEAM_SUM, K_WIN_ROW_FFT, K_WIN_COL_ABS2, K_BIN_REDUCE, K_COL_MS_INIT, K_COL_MS_FINAL,
-                   K_LATTICE_DFT, K_PATTERNS, K_DETECTORS, K_NUM_CLASSES };
+                   K_LATTICE_DFT, K_PATTERNS, K_DETECTORS, K_ACCUMULATE, K_NUM_CLASSES };
 static const char* const kClassNames[K_NUM_CLASSES] = {
     "potential", "transmission", "row_init", "row_step", "row_final", "col_step", "beam_sum",
-    "win_row_fft", "win_col_abs2", "bin_reduce", "col_ms_init", "col_ms_final", "lattice_dft", "patterns", "detectors" };
+    "win_row_fft", "win_col_abs2", "bin_reduce", "col_ms_init", "col_ms_final", "lattice_dft", "patterns", "detectors", "accumulate" };
 struct TimedLaunch { int cls; cudaEvent_t e0, e1; };
-static bool g_timing = false;
+// The record is process-wide and guarded by a mutex that is taken only while timing is enabled.
+static std::atomic<bool> g_timing{false};
+static std::mutex g_timing_mu;
 static std::vector<TimedLaunch> g_timed;
 static std::vector<cudaEvent_t> g_event_pool;      // events are reused: creating them costs more than recording
 static cudaEvent_t take_event()
 {
+    std::lock_guard<std::mutex> lock(g_timing_mu);
     cudaEvent_t e = nullptr;
     if (!g_event_pool.empty()) { e = g_event_pool.back(); g_event_pool.pop_back(); }
     else cudaEventCreate(&e);
     return e;
 }
+static void record_timed(int cls, cudaEvent_t e0, cudaEvent_t e1)
+{
+    std::lock_guard<std::mutex> lock(g_timing_mu);
+    g_timed.push_back({cls, e0, e1});
+}
 
 #define LAUNCH(cls, call, stream)                                                      \
     do {                                                                               \
         cudaEvent_t e0__ = nullptr, e1__ = nullptr;                                    \
-        if (g_timing) {                                                                \
+        const bool timed__ = g_timing.load(std::memory_order_relaxed);                 \
+        if (timed__) {                                                                 \
             e0__ = take_event(); e1__ = take_event();                                  \
             cudaEventRecord(e0__, (stream));                                           \
         }                                                                              \
         cudaError_t e__ = (call);                                                      \
         if (e__ != cudaSuccess) return cuda_fail(e__, #call);                          \
-        if (g_timing) { cudaEventRecord(e1__, (stream)); g_timed.push_back({(cls), e0__, e1__}); } \
+        if (timed__) { cudaEventRecord(e1__, (stream)); record_timed((cls), e0__, e1__); } \
         g_launches.fetch_add(1, std::memory_order_relaxed);                            \
     } while (0)
 
@@ -589,9 +599,7 @@ int64_t prism_launch_count(int32_t reset)
 
 int32_t prism_timing_enable(int32_t enable)
 {
-    const int32_t was = g_timing ? 1 : 0;
-    g_timing = enable != 0;
-    return was;
+    return g_timing.exchange(enable != 0) ? 1 : 0;
 }
 
 int32_t prism_timing_classes(void) { return K_NUM_CLASSES; }
@@ -601,6 +609,7 @@ int prism_timing_read(double* ms_by_class, int64_t* launches_by_class)
 {
     if (!ms_by_class || !launches_by_class) return PRISM_EINVAL;
     for (int c = 0; c < K_NUM_CLASSES; ++c) { ms_by_class[c] = 0.0; launches_by_class[c] = 0; }
+    std::lock_guard<std::mutex> lock(g_timing_mu);
     for (const TimedLaunch& t : g_timed) {
         CU(cudaEventSynchronize(t.e1));
         float ms = 0.f;
@@ -611,6 +620,15 @@ int prism_timing_read(double* ms_by_class, int64_t* launches_by_class)
         g_event_pool.push_back(t.e1);
     }
     g_timed.clear();
+    return PRISM_OK;
+}
+
+int prism_accumulate(float* acc, const float* x, int64_t n, float weight, int32_t first, void* cuda_stream)
+{
+    if (!acc || !x || n < 0) return PRISM_EINVAL;
+    if (!pointer_is_device(acc) || !pointer_is_device(x)) return PRISM_EINVAL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    LAUNCH(K_ACCUMULATE, launch_accumulate(acc, x, n, weight, first != 0, st), st);
     return PRISM_OK;
 }
 

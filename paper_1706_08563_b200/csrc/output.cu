@@ -77,11 +77,9 @@ cudaError_t launch_beam_sum(const BeamSumArgs& g, cudaStream_t stream)
     threads = ((threads + 31) / 32) * 32;
     if (threads > 1024) return cudaErrorInvalidValue;       // windows up to 128 x 128
     const size_t smem = (size_t)g.n_beams * sizeof(float2);
-    if (smem > 48 * 1024) {
-        static bool set = false;
-        if (!set) { cudaFuncSetAttribute(beam_sum_kernel<BEAM_SUM_PPT>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024); set = true; }
-        if (smem > 200 * 1024) return cudaErrorInvalidValue;
-    }
+    if (smem > 200 * 1024) return cudaErrorInvalidValue;
+    static PerDevice once{};
+    if (cudaError_t e = opt_in_smem(beam_sum_kernel<BEAM_SUM_PPT>, 200 * 1024, once); e != cudaSuccess) return e;
     beam_sum_kernel<BEAM_SUM_PPT><<<g.n_probes_batch, threads, smem, stream>>>(g);
     return cudaGetLastError();
 }
@@ -200,12 +198,8 @@ template <int Q>
 static cudaError_t launch_lattice_q(const LatticeArgs& g, cudaStream_t stream)
 {
     using C = LatticeCfg<Q>;
-    static bool set = false;
-    if (!set) {
-        cudaError_t e = cudaFuncSetAttribute(lattice_dft_kernel<Q>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
-        if (e != cudaSuccess) return e;
-        set = true;
-    }
+    static PerDevice once{};
+    if (cudaError_t e = opt_in_smem(lattice_dft_kernel<Q>, C::SMEM, once); e != cudaSuccess) return e;
     if (g.nx % C::TP) return cudaErrorInvalidValue;
     const long long blocks = (long long)(g.nx / C::TP) * g.n_pix_rows;
     if (blocks <= 0) return cudaSuccess;
@@ -354,6 +348,25 @@ cudaError_t launch_mask_dot(const float* intensity, const float* masks, int n_ma
     else if (n_masks <= 4) mask_dot_kernel<4><<<n_waves, 256, 0, stream>>>(intensity, masks, n_masks, mx, my, out);
     else if (n_masks <= 8) mask_dot_kernel<8><<<n_waves, 256, 0, stream>>>(intensity, masks, n_masks, mx, my, out);
     else                   mask_dot_kernel<16><<<n_waves, 256, 0, stream>>>(intensity, masks, n_masks, mx, my, out);
+    return cudaGetLastError();
+}
+
+// Frozen-phonon accumulation: acc = (first ? 0 : acc) + weight * x, element by element.
+__global__ void __launch_bounds__(256) accumulate_kernel(float* __restrict__ acc, const float* __restrict__ x,
+                                                         int64_t n, float weight, int first)
+{
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride)
+        acc[i] = first ? weight * x[i] : fmaf(weight, x[i], acc[i]);
+}
+
+cudaError_t launch_accumulate(float* acc, const float* x, int64_t n, float weight, bool first, cudaStream_t stream)
+{
+    if (n <= 0) return cudaSuccess;
+    long long blocks = (n + 255) / 256;
+    const long long cap = (long long)num_sms() * 8;
+    if (blocks > cap) blocks = cap;
+    accumulate_kernel<<<(unsigned)blocks, 256, 0, stream>>>(acc, x, n, weight, first ? 1 : 0);
     return cudaGetLastError();
 }
 

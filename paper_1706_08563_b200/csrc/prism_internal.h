@@ -5,7 +5,48 @@
 #include <stddef.h>
 #include <stdint.h>
 
+#include <atomic>
+
 namespace prism {
+
+// ---- per-device launch set-up -----------------------------------------------------
+// Function attributes (the opt-in to more than 48 KiB of dynamic shared memory) and occupancy results belong to
+// a device, so "already done" is remembered per device.  The marks are idempotent: two host threads racing on the
+// same mark both do the (identical) set-up.
+constexpr int MAX_DEVICES = 64;
+inline int current_device()
+{
+    int d = 0;
+    if (cudaGetDevice(&d) != cudaSuccess || d < 0 || d >= MAX_DEVICES) d = 0;
+    return d;
+}
+struct PerDevice { std::atomic<int> v[MAX_DEVICES]; };
+template <class K>
+inline cudaError_t opt_in_smem(K kern, size_t smem, PerDevice& once)
+{
+    const int d = current_device();
+    if (once.v[d].load(std::memory_order_acquire)) return cudaSuccess;
+    if (smem > 48 * 1024) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+    }
+    once.v[d].store(1, std::memory_order_release);
+    return cudaSuccess;
+}
+// resident CTAs per SM of `kern` at this launch shape on the current device (after the shared-memory opt-in)
+template <class K>
+inline int blocks_per_sm_cached(K kern, int threads, size_t smem, PerDevice& cache)
+{
+    const int d = current_device();
+    int n = cache.v[d].load(std::memory_order_acquire);
+    if (n > 0) return n;
+    if (smem > 48 * 1024) cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    n = 0;
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, kern, threads, smem);
+    if (n <= 0) n = 1;
+    cache.v[d].store(n, std::memory_order_release);
+    return n;
+}
 
 // ---- slice-step passes (slice_pass.cu) -----------------------------------------
 // Waves live in "mixed space" A[w][y][kx] = sum_x psi[w][y][x] exp(-2 pi i kx x / nx)
@@ -116,6 +157,10 @@ cudaError_t launch_transpose_patterns(const float* intensity, float* patterns, i
 // out[w][d] = sum over pixels of masks[d][ky][kx] * intensity[w][kx][ky], d < n_masks <= 16 (virtual detectors)
 cudaError_t launch_mask_dot(const float* intensity, const float* masks, int n_masks, int mx, int my, float* out,
                             int n_waves, cudaStream_t stream);
+
+// acc = (first ? 0 : acc) + weight * x   (frozen-phonon accumulation)
+cudaError_t launch_accumulate(float* acc, const float* x, int64_t n, float weight, bool first, cudaStream_t stream);
+int num_sms();
 
 // ---- potential (potential.cu) ------------------------------------------------------
 struct PotAtom { double x, y; int32_t lut; int32_t pad; };

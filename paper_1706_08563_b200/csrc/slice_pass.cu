@@ -16,16 +16,17 @@
 
 namespace prism {
 
-static int g_num_sms = 0;
 int num_sms()
 {
-    if (!g_num_sms) {
-        int dev = 0;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&g_num_sms, cudaDevAttrMultiProcessorCount, dev);
-        if (g_num_sms <= 0) g_num_sms = 148;
+    static PerDevice cache{};
+    const int d = current_device();
+    int n = cache.v[d].load(std::memory_order_acquire);
+    if (n <= 0) {
+        cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, d);
+        if (n <= 0) n = 148;
+        cache.v[d].store(n, std::memory_order_release);
     }
-    return g_num_sms;
+    return n;
 }
 
 __device__ __forceinline__ void cp_async8(void* smem_dst, const void* gmem_src)
@@ -103,12 +104,8 @@ static cudaError_t launch_row_t(const RowArgs& g, cudaStream_t stream)
     auto kern = row_pass_kernel<P, LPC, MODE>;
     const int threads = P::T * LPC;
     const size_t smem = (size_t)LPC * P::PADDED * sizeof(float2);
-    static int blocks_per_sm = 0;
-    if (!blocks_per_sm) {
-        if (smem > 48 * 1024) cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks_per_sm, kern, threads, smem);
-        if (blocks_per_sm <= 0) blocks_per_sm = 1;
-    }
+    static PerDevice occupancy{};
+    const int blocks_per_sm = blocks_per_sm_cached(kern, threads, smem, occupancy);
     const long long n_lines = (long long)g.n_waves * g.ny;
     const long long n_groups = (n_lines + LPC - 1) / LPC;
     if (n_groups == 0) return cudaSuccess;
@@ -250,12 +247,8 @@ static cudaError_t launch_col_t(const ColArgs& g, cudaStream_t stream)
     auto kern = col_pass_kernel<P, W, G, MODE>;
     const int threads = (W / G) * P::T;
     const size_t smem = (size_t)P::PADDED * (W + 1) * sizeof(float2);
-    static int blocks_per_sm = 0;
-    if (!blocks_per_sm) {
-        if (smem > 48 * 1024) cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks_per_sm, kern, threads, smem);
-        if (blocks_per_sm <= 0) blocks_per_sm = 1;
-    }
+    static PerDevice occupancy{};
+    const int blocks_per_sm = blocks_per_sm_cached(kern, threads, smem, occupancy);
     const long long n_tiles = (long long)g.n_waves * (g.nx / W);
     if (n_tiles == 0) return cudaSuccess;
     long long grid = (long long)num_sms() * blocks_per_sm;

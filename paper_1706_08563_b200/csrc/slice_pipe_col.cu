@@ -150,9 +150,7 @@ __global__ void __launch_bounds__(ColCfg<P>::THREADS, 1) col_pipe_kernel(ColArgs
 #pragma unroll
             for (int e = 0; e < E; ++e) v[e] = sm.ld(t + T * e);
             fft_forward<P>(v, tw, t, sm);
-            // Fresnel propagator with the 2/3 band-limit (Eq. 2; BASELINE.json): the table holds
-            // prop_x[kx] prop_y[ky] inside the band and zero outside, [ky][kx] like the wave (L2 resident)
-// Fresnel propagator with the 2/3 band-limit (Eq. 2; BASELINE.json).  With YBE > 0 the
+            // Fresnel propagator with the 2/3 band-limit (Eq. 2; BASELINE.json).  With YBE > 0 the
             // register slots e in [YBE, E - YBE) hold |ky| beyond every column's limit: zero without any work.
             const float2 pxv = __ldg(g.prop_x + kxi);
             const int lim = __ldg(g.ky_lim + kxi);
@@ -199,12 +197,8 @@ static cudaError_t launch_col_pipe_s(const ColArgs& g, cudaStream_t stream)
 {
     using C = ColCfg<P>;
     auto kern = col_pipe_kernel<P, MODE, SQ, YBE>;
-    static bool set = false;
-    if (!set) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
-        if (e != cudaSuccess) return e;
-        set = true;
-    }
+    static PerDevice once{};
+    if (cudaError_t e = opt_in_smem(kern, C::SMEM, once); e != cudaSuccess) return e;
     if (g.xband % C::W || g.nx % C::W) return cudaErrorInvalidValue;
     const long long n_items = (long long)g.n_waves * (2 * g.xband / C::W);
     if (n_items == 0) return cudaSuccess;

@@ -188,12 +188,8 @@ static cudaError_t launch_row_pipe_x(const RowArgs& g, cudaStream_t stream)
 {
     using C = RowCfg<P, XBE>;
     auto kern = row_pipe_kernel<P, MODE, XBE>;
-    static bool set = false;
-    if (!set) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
-        if (e != cudaSuccess) return e;
-        set = true;
-    }
+    static PerDevice once{};
+    if (cudaError_t e = opt_in_smem(kern, C::SMEM, once); e != cudaSuccess) return e;
     const long long n_lines = (long long)g.n_waves * g.ny;
     const long long n_groups = (n_lines + C::LPT - 1) / C::LPT;
     if (n_groups == 0) return cudaSuccess;

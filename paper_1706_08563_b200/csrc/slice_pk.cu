@@ -185,12 +185,8 @@ static cudaError_t launch_row_pk_x(const RowArgs& g, cudaStream_t stream)
 {
     using C = RowPkCfg<N, XBE>;
     auto kern = row_pk_kernel<N, MODE, XBE>;
-    static bool set = false;
-    if (!set) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
-        if (e != cudaSuccess) return e;
-        set = true;
-    }
+    static PerDevice once{};
+    if (cudaError_t e = opt_in_smem(kern, C::SMEM, once); e != cudaSuccess) return e;
     const long long n_lines = (long long)g.n_waves * g.ny;
     const long long n_groups = (n_lines + C::LPW - 1) / C::LPW;
     if (n_groups == 0) return cudaSuccess;
@@ -404,12 +400,8 @@ static cudaError_t launch_col_pk_s(const ColArgs& g, cudaStream_t stream)
 {
     using C = ColPkCfg<N>;
     auto kern = col_pk_kernel<N, MODE, SQ, YBE>;
-    static bool set = false;
-    if (!set) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)C::SMEM);
-        if (e != cudaSuccess) return e;
-        set = true;
-    }
+    static PerDevice once{};
+    if (cudaError_t e = opt_in_smem(kern, C::SMEM, once); e != cudaSuccess) return e;
     if (g.xband % C::W || g.nx % C::W) return cudaErrorInvalidValue;
     const long long n_items = (long long)g.n_waves * (2 * g.xband / C::W);
     if (n_items == 0) return cudaSuccess;

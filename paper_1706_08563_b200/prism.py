@@ -21,7 +21,7 @@ WS_SMATRIX, WS_OUTPUT, WS_MULTISLICE, WS_POTENTIAL = 0, 1, 2, 3
 EXPORTS = ["prism_workspace_bytes", "prism_num_bins", "prism_num_beams", "prism_band_columns", "prism_constants",
            "prism_build_potential", "prism_compute_smatrix", "prism_compute_output",
            "multislice_compute_output", "prism_compute_patterns", "multislice_compute_patterns",
-           "prism_compute_detectors", "multislice_compute_detectors", "prism_strerror", "prism_last_error", "prism_launch_count",
+           "prism_compute_detectors", "multislice_compute_detectors", "prism_accumulate", "prism_strerror", "prism_last_error", "prism_launch_count",
            "prism_timing_enable", "prism_timing_classes", "prism_timing_class_name", "prism_timing_read"]
 
 
@@ -84,6 +84,8 @@ def _load() -> C.CDLL:
     lib.prism_compute_detectors.argtypes = [pp, vp, vp, i32, vp, i32, vp, vp, sz, vp]
     lib.multislice_compute_detectors.restype = C.c_int
     lib.multislice_compute_detectors.argtypes = [pp, vp, vp, i32, vp, vp, sz, vp]
+    lib.prism_accumulate.restype = C.c_int
+    lib.prism_accumulate.argtypes = [vp, vp, i64, C.c_float, i32, vp]
     lib.prism_strerror.restype = C.c_char_p
     lib.prism_strerror.argtypes = [C.c_int]
     lib.prism_last_error.restype = C.c_char_p
@@ -219,6 +221,14 @@ def multislice_output(p: Params, v, out, workspace, stream=None):
                                           workspace.numel() * workspace.element_size(), _stream_ptr(stream)),
            "multislice_compute_output")
     return out
+
+
+def accumulate(acc, x, weight: float = 1.0, first: bool = False, stream=None):
+    """``prism_accumulate``: acc = (first ? 0 : acc) + weight * x on CUDA fp32 tensors of equal size."""
+    assert acc.numel() == x.numel()
+    _check(_lib.prism_accumulate(_ptr(acc), _ptr(x), acc.numel(), float(weight), 1 if first else 0,
+                                 _stream_ptr(stream)), "prism_accumulate")
+    return acc
 
 
 def compute_patterns(p: Params, s, beams, patterns, workspace, stream=None):

@@ -12,6 +12,14 @@ def phonons_for_rank(n_phonons: int, world: int, rank: int) -> list[int]:
     return [ph for ph in range(max(n_phonons, world)) if ph % world == rank]
 
 
+def all_reduce_sum(acc, dist=None):
+    """Sum of `acc` over ranks, in place (a collective, no arithmetic here): with every rank accumulating its
+    configurations through ``prism_accumulate`` at weight 1 / (total configurations), the result is the mean."""
+    if dist is not None and dist.is_initialized() and dist.get_world_size() > 1:
+        dist.all_reduce(acc)
+    return acc
+
+
 def phonon_average(acc, count: int, dist=None):
     """Mean over all configurations of all ranks: acc holds this rank's sum of `count` outputs (a torch tensor,
     reduced in place).  dist: an initialised torch.distributed module, or None for a single process."""

@@ -100,6 +100,38 @@ def test_multislice_parity(G, name):
     assert rel_l2(out[:, d:], ref[:, d:]) < 5 * TOL_OUT
 
 
+def test_frozen_phonon_average_parity(G):
+    """Row FP of SURVEY.md 8(a) (images are averaged over frozen-phonon configurations): three
+    thermally displaced configurations of a 128^2 case, each a full GPU run atoms -> rings, averaged on the device
+    by prism_accumulate; against the mean of the oracle's three full runs."""
+    from paper_1706_08563_b200 import prism
+    w = W.scaled_test_case(128, 4, 2, 6, alpha_mrad=25.0, defocus=25.0, seed_index=21, density=0.25,
+                           z_choices=(79, 33, 14), probe_offset=(0.05, 0.11)).with_(jitter=0.08, n_phonons=3)
+    p = oracle_params(w)
+    pp = prism.params_from_workload(w)
+    n_bins = prism.num_bins(pp)
+    acc = torch.full((w.probes_y, w.probes_x, n_bins), float("nan"), dtype=torch.float32, device=G.DEV)
+    out = torch.empty_like(acc)
+    refs, singles = [], []
+    for ph in range(w.n_phonons):
+        v = G.gpu_potential(w, phonon=ph)
+        s, beams = G.gpu_smatrix(w, v)
+        prism.compute_output(pp, s, beams, out, G.ws(pp, prism.WS_OUTPUT))
+        prism.accumulate(acc, out, 1.0 / w.n_phonons, first=(ph == 0))
+        singles.append(out.cpu().numpy().astype(np.float64).reshape(-1, n_bins))
+        v_ref = oracle_potential(w, phonon=ph)
+        refs.append(O.prism_probes(p, O.smatrix(p, v_ref, beams), beams, w.probe_xy()))
+    torch.cuda.synchronize()
+    got = acc.cpu().numpy().astype(np.float64).reshape(-1, n_bins)
+    ref = np.mean(refs, axis=0)
+    assert rel_l2(got, ref) < TOL_OUT
+    d = G.dark_field(w, p)
+    assert rel_l2(got[:, d:], ref[:, d:]) < 5 * TOL_OUT
+    # the configurations differ, so the mean is not any single run (the test would pass trivially otherwise)
+    assert rel_l2(singles[0], ref) > 20 * TOL_OUT
+    assert np.allclose(got, np.mean(singles, axis=0), rtol=1e-5, atol=1e-10)
+
+
 # ---- regular probe lattices: the lattice-DFT form of the beam sum (DESIGN.md section 7) -----------------
 def _lattice_cases():
     return {
