@@ -430,13 +430,19 @@ static int smatrix_batch(const prism_params* p, int n_beams)
     const long long per_beam = (long long)p->nx * p->ny * (long long)sizeof(float2);
     return (int)std::max<long long>(1, std::min<long long>(n_beams, (long long)(8ull << 30) / per_beam));
 }
-struct SmatrixLayout { SliceTables tab; SliceFeeder feed; int2* beams; float2* wave; };
+// Grids on the blocked mixed-space layout (blocked_grid): the last row pass turns blocked mixed space into natural
+// real space, which cannot be done in place, so it runs FINAL_CHUNK waves at a time into a staging buffer that is
+// then copied over the waves' own storage (or straight to a host S-matrix).
+constexpr int FINAL_CHUNK = 16;
+struct SmatrixLayout { SliceTables tab; SliceFeeder feed; int2* beams; float2* wave; float2* final_stage; int final_chunk; };
 static void layout_smatrix(Arena& a, const prism_params* p, int n_beams, SmatrixLayout& L)
 {
     carve_slice_tables(a, p, L.tab);
     carve_feeder(a, p, L.feed, p->smatrix_on_host != 0 && smatrix_batch(p, n_beams) < n_beams);
     L.beams = a.take<int2>(n_beams);
     L.wave = p->smatrix_on_host ? a.take<float2>((size_t)smatrix_batch(p, n_beams) * p->nx * p->ny) : nullptr;
+    L.final_chunk = blocked_grid(p->nx, p->ny) ? std::min(FINAL_CHUNK, std::max(1, n_beams)) : 0;
+    L.final_stage = L.final_chunk ? a.take<float2>((size_t)L.final_chunk * p->nx * p->ny) : nullptr;
 }
 
 constexpr int LATTICE_MAX_SLOTS = 4, LATTICE_MAX_Q = 32;
@@ -830,6 +836,7 @@ int prism_compute_smatrix(const prism_params* p, const float* v, int32_t* beams_
 
     const int batch = smatrix_batch(p, n_beams);
     const bool s_on_host = p->smatrix_on_host != 0;
+    const bool blocked = blocked_grid(p->nx, p->ny);
     auto run = [&]() -> int {
         for (int b0 = 0; b0 < n_beams; b0 += batch) {
             const int nb = std::min(batch, n_beams - b0);
@@ -838,9 +845,10 @@ int prism_compute_smatrix(const prism_params* p, const float* v, int32_t* beams_
             ra.a = s_on_host ? L.wave : (float2*)s + (size_t)b0 * npix; ra.out = ra.a; ra.t = feed.tbuf;
             ra.tw_x = L.tab.tw_x; ra.tw_y = L.tab.tw_y; ra.beams = L.beams + b0;
             ra.n_waves = nb; ra.nx = p->nx; ra.ny = p->ny; ra.scale = 1.f; ra.xband = xband;
+            ra.blocked = blocked ? 1 : 0;
             ColArgs ca;
             std::memset(&ca, 0, sizeof(ca));
-            ca.xband = xband; ca.yband = yband;
+            ca.xband = xband; ca.yband = yband; ca.blocked = ra.blocked;
             ca.a = ra.a; ca.tw_y = L.tab.tw_y; ca.prop_x = L.tab.prop_x; ca.prop_y = L.tab.prop_y;
             ca.ky_lim = L.tab.ky_lim; ca.n_waves = nb; ca.nx = p->nx; ca.ny = p->ny; ca.scale = 1.f;
             feed.begin_sweep();
@@ -857,10 +865,26 @@ int prism_compute_smatrix(const prism_params* p, const float* v, int32_t* beams_
                 LAUNCH(K_COL_STEP, launch_col_pass(COL_STEP, ca, st), st);
             }
             ra.scale = 1.0f / (float)p->nx;
-            LAUNCH(K_ROW_FINAL, launch_row_pass(ROW_FINAL, ra, st), st);
-            if (s_on_host)
-                CU(cudaMemcpyAsync((float2*)s + (size_t)b0 * npix, L.wave, (size_t)nb * npix * sizeof(float2),
-                                   cudaMemcpyDeviceToHost, st));
+            if (!blocked) {
+                LAUNCH(K_ROW_FINAL, launch_row_pass(ROW_FINAL, ra, st), st);
+                if (s_on_host)
+                    CU(cudaMemcpyAsync((float2*)s + (size_t)b0 * npix, L.wave, (size_t)nb * npix * sizeof(float2),
+                                       cudaMemcpyDeviceToHost, st));
+            } else {
+                // blocked mixed space -> natural real space through the staging buffer, a few waves at a time
+                for (int c0 = 0; c0 < nb; c0 += L.final_chunk) {
+                    const int nc = std::min(L.final_chunk, nb - c0);
+                    RowArgs rf = ra;
+                    rf.a = ra.a + (size_t)c0 * npix; rf.out = L.final_stage; rf.n_waves = nc;
+                    LAUNCH(K_ROW_FINAL, launch_row_pass(ROW_FINAL, rf, st), st);
+                    if (s_on_host)
+                        CU(cudaMemcpyAsync((float2*)s + (size_t)(b0 + c0) * npix, L.final_stage,
+                                           (size_t)nc * npix * sizeof(float2), cudaMemcpyDeviceToHost, st));
+                    else
+                        CU(cudaMemcpyAsync(rf.a, L.final_stage, (size_t)nc * npix * sizeof(float2),
+                                           cudaMemcpyDeviceToDevice, st));
+                }
+            }
         }
         return PRISM_OK;
     };
@@ -1141,11 +1165,12 @@ static int multislice_impl(const prism_params* p, const float* v, float* out, fl
             ca.prop_y = L.tab.prop_y; ca.ky_lim = L.tab.ky_lim; ca.aperture_t = L.aperture_t;
             ca.phase_x = L.phase_x; ca.phase_y = L.phase_y; ca.probe0 = p0; ca.probes_x = p->probes_x;
             ca.n_waves = np; ca.nx = nx; ca.ny = ny; ca.xband = xband; ca.yband = band_rows(p);
+            ca.blocked = blocked_grid(nx, ny) ? 1 : 0;
             ca.scale = (float)((double)ny / (double)nx);      // I = |Psi_S|^2 / (nx ny), see DESIGN.md
             RowArgs ra;
             std::memset(&ra, 0, sizeof(ra));
             ra.a = L.psi; ra.out = L.psi; ra.t = feed.tbuf; ra.tw_x = L.tab.tw_x; ra.tw_y = L.tab.tw_y;
-            ra.n_waves = np; ra.nx = nx; ra.ny = ny; ra.scale = 1.f; ra.xband = xband;
+            ra.n_waves = np; ra.nx = nx; ra.ny = ny; ra.scale = 1.f; ra.xband = xband; ra.blocked = ca.blocked;
             LAUNCH(K_COL_MS_INIT, launch_col_pass(COL_MS_INIT, ca, st), st);
             feed.begin_sweep();
             for (int sl = 0; sl < p->n_slices; ++sl) {

@@ -67,6 +67,8 @@ struct RowArgs {
     int           n_waves, nx, ny;
     int           xband;      // mixed space is read / written for kx in [0, xband) and [nx - xband, nx) only
                               // (pipelined kernels; everything outside is zero by the 2/3 band-limit)
+    int           blocked;    // 1: mixed space in the blocked layout "B8" (blocked_grid(); slice_pk.cu); ROW_FINAL then
+                              // needs out != a (real space is natural order: the layouts differ, no in-place pass)
     float         scale;      // ROW_INIT: plane-wave amplitude; ROW_FINAL: output scale
 };
 cudaError_t launch_row_pass(RowMode mode, const RowArgs& args, cudaStream_t stream);
@@ -77,6 +79,12 @@ cudaError_t launch_row_pipe(RowMode mode, const RowArgs& args, cudaStream_t stre
 // stored in pair layout t[y][j] = (re(2j), re(2j+1), im(2j), im(2j+1))
 inline bool packed_row(int nx, int ny) { return pipelined_grid(nx, ny) && nx == 2048; }
 cudaError_t launch_row_pk(RowMode mode, const RowArgs& args, cudaStream_t stream);
+// grids whose mixed space uses the blocked layout "B8" (slice_pk.cu): tiles of 8 in-band columns, each tile
+// [ny][8] contiguous, so that the 2048-point column pass moves 128 KB runs instead of 32-byte row segments
+#ifndef PRISM_BLOCKED_LAYOUT
+#define PRISM_BLOCKED_LAYOUT 1
+#endif
+inline bool blocked_grid(int nx, int ny) { return PRISM_BLOCKED_LAYOUT && nx == 2048 && ny == 2048; }
 
 enum ColMode {
     COL_STEP     = 0,   // A -> FFT_y -> * P -> IFFT_y -> A
@@ -99,6 +107,7 @@ struct ColArgs {
     int           n_waves, nx, ny;
     int           xband;      // see RowArgs
     int           yband;      // a multiple of 32 with ky_lim[kx] < yband for every kx (pipelined kernels)
+    int           blocked;    // 1: mixed space in the blocked layout "B8" (see RowArgs)
     float         scale;      // COL_ABS2 / COL_MS_FINAL intensity scale
 };
 cudaError_t launch_col_pass(ColMode mode, const ColArgs& args, cudaStream_t stream);

@@ -15,10 +15,23 @@
 //
 // so global memory is always read and written in natural order with coalesced accesses and no register
 // shuffling is needed between the pair layout and memory.
+//
+// Blocked mixed space "B8" (square 2048-point grids; prism_internal.h `blocked_grid`): between the two passes a
+// wave holds only its 2 xb in-band columns, in compact order j (j < xb: kx = j; j >= xb: slot nx - 2 xb + j), as
+// tiles of 8 columns,   element (y, j) at  a[w nx ny + ((j >> 3) ny + y) 8 + (j & 7)],
+// so that a column tile [ny rows] x [8 columns] is ONE contiguous 128 KB run: the column pass fetches it with a
+// few bulk copies (no LSU work) and stores it back from registers as 256-byte runs (4 rows x 64 B per warp
+// instruction) instead of 32-byte row segments; the row pass gathers a line as 2 xb / 8 pieces of 64 bytes
+// (one 4-D TMA tensor box, or 16-byte cp.async copies) and stores 4 x 64 B per warp instruction.
+#include <cuda.h>
+
 #include "fft_core.cuh"
 #include "fft_pk.cuh"
 #include "pipe_ptx.cuh"
 #include "prism_internal.h"
+
+#include <atomic>
+#include <cstring>
 
 namespace prism {
 
@@ -47,8 +60,18 @@ struct RowPkCfg {
     static constexpr size_t SMEM = PIPE_HEADER + TWB + (size_t)WARPS * PER_WARP;
 };
 
-template <int N, int MODE, int XBE>
-__global__ void __launch_bounds__(RowPkCfg<N, XBE>::THREADS, 1) row_pk_kernel(RowArgs g)
+// LAYOUT of mixed space: LAY_NATURAL a[w][y][kx]; LAY_B8_CPA / LAY_B8_TMA blocked "B8" (see the top of this file),
+// the line gathered by 16-byte cp.async copies of all lanes / by one 4-D TMA tensor box {8, 1, 2 xb / 8, 1}.
+enum { LAY_NATURAL = 0, LAY_B8_CPA = 1, LAY_B8_TMA = 2 };
+__device__ __forceinline__ void tensor_g2s_4d(void* smem_dst, const CUtensorMap* map, int c0, int c1, int c2, int c3,
+                                              uint64_t* bar)
+{
+    asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
+                 ::"r"(smem_u32(smem_dst)), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(smem_u32(bar)) : "memory");
+}
+
+template <int N, int MODE, int XBE, int LAYOUT>
+__global__ void __launch_bounds__(RowPkCfg<N, XBE>::THREADS, 1) row_pk_kernel(RowArgs g, const __grid_constant__ CUtensorMap tmap)
 {
     using C = RowPkCfg<N, XBE>;
     using P = typename C::P;
@@ -63,18 +86,36 @@ __global__ void __launch_bounds__(RowPkCfg<N, XBE>::THREADS, 1) row_pk_kernel(Ro
     float2* xch = reinterpret_cast<float2*>(mine + C::LAND_BYTES);             // [LPW][XPAD]
 
     pk::fill_tables<P>(tab, g.tw_x, tid, C::THREADS);
-    if (MODE != ROW_INIT && lane == 0) { mbar_init(&bars[warp], 1); mbar_fence_init(); }
+    if (MODE != ROW_INIT && lane == 0) { mbar_init(&bars[warp], LAYOUT == LAY_B8_CPA ? 32 : 1); mbar_fence_init(); }
     __syncthreads();
     griddep_wait();                          // the previous kernel of the slice loop has completed (pipe_ptx.cuh)
     griddep_launch();
 
+    const size_t wave_stride = (size_t)g.ny * N;
     const long long n_lines = (long long)g.n_waves * g.ny;
     const long long n_groups = (n_lines + LPW - 1) / LPW;
     const long long gw = (long long)blockIdx.x * C::WARPS + warp, gstride = (long long)gridDim.x * C::WARPS;
     const int xb = XBE < 32 ? XBE * T : g.xband;                 // in-band columns: [0, xb) and [N - xb, N)
 
-    // lane 0: start the bulk copies of line group `grp` into the landing buffer
+    // start the copies of line group `grp` into the landing buffer (compact: [0, xb) then [N - xb, N)).
+    // LAY_B8_CPA: called by every lane of the warp; otherwise by lane 0 only.
     auto issue = [&](long long grp) {
+        if (LAYOUT == LAY_B8_CPA) {
+#pragma unroll
+            for (int l = 0; l < LPW; ++l) {
+                const long long line = grp * LPW + l;
+                if (line < n_lines) {
+                    const int y = (int)(line / g.n_waves), w = (int)(line % g.n_waves);
+                    const float2* src = g.a + (size_t)w * wave_stride + (size_t)y * 8;
+                    float2* dst = land + l * C::LANDW;
+                    // 16-byte chunk q of the compact line: piece q / 4 (64 bytes of tile q / 4), quarter q % 4
+                    for (int q = lane; q < xb; q += 32)
+                        cp_async16(dst + 2 * q, src + (size_t)(q >> 2) * g.ny * 8 + 2 * (q & 3));
+                }
+            }
+            cp_async_arrive(&bars[warp]);
+            return;
+        }
         int n_act = 0;
 #pragma unroll
         for (int l = 0; l < LPW; ++l) n_act += (grp * LPW + l < n_lines);
@@ -84,14 +125,18 @@ __global__ void __launch_bounds__(RowPkCfg<N, XBE>::THREADS, 1) row_pk_kernel(Ro
             const long long line = grp * LPW + l;
             if (line < n_lines) {
                 const int y = (int)(line / g.n_waves), w = (int)(line % g.n_waves);
-                const float2* row = g.a + ((size_t)w * g.ny + y) * N;
                 float2* dst = land + l * C::LANDW;
-                bulk_g2s(dst, row, (unsigned)(xb * sizeof(float2)), &bars[warp]);
-                bulk_g2s(dst + xb, row + (N - xb), (unsigned)(xb * sizeof(float2)), &bars[warp]);
+                if (LAYOUT == LAY_B8_TMA) {
+                    tensor_g2s_4d(dst, &tmap, 0, y, 0, w, &bars[warp]);
+                } else {
+                    const float2* row = g.a + ((size_t)w * g.ny + y) * N;
+                    bulk_g2s(dst, row, (unsigned)(xb * sizeof(float2)), &bars[warp]);
+                    bulk_g2s(dst + xb, row + (N - xb), (unsigned)(xb * sizeof(float2)), &bars[warp]);
+                }
             }
         }
     };
-    if (MODE != ROW_INIT && lane == 0 && gw < n_groups) issue(gw);
+    if (MODE != ROW_INIT && (LAYOUT == LAY_B8_CPA || lane == 0) && gw < n_groups) issue(gw);
 
     const pk::XchgPhase sm{ xch + ll * P::XPAD, 1 };
     auto sync = [] { __syncwarp(); };
@@ -103,7 +148,8 @@ __global__ void __launch_bounds__(RowPkCfg<N, XBE>::THREADS, 1) row_pk_kernel(Ro
         const bool active = line < n_lines;
         if (!active) line = n_lines - 1;                 // keep every lane in the warp barriers
         const int y = (int)(line / g.n_waves), w = (int)(line % g.n_waves);
-        float2* row = g.a + ((size_t)w * g.ny + y) * N;
+        // natural: the row itself; blocked: row y of tile 0 of the wave (column j lives (j >> 3) ny 8 + (j & 7) further on)
+        float2* row = LAYOUT == LAY_NATURAL ? g.a + ((size_t)w * g.ny + y) * N : g.a + (size_t)w * wave_stride + (size_t)y * 8;
         C2 p[32];
 
         // Phase 0 builds the pairs the first half-length transform runs on (plane wave, or the landed line after
@@ -128,7 +174,8 @@ __global__ void __launch_bounds__(RowPkCfg<N, XBE>::THREADS, 1) row_pk_kernel(Ro
                 }
                 // the landing buffer is free once every lane has read its points
                 __syncwarp();
-                if (lane == 0 && grp + gstride < n_groups) { fence_proxy_async(); issue(grp + gstride); }
+                if (LAYOUT == LAY_B8_CPA) { if (grp + gstride < n_groups) issue(grp + gstride); }
+                else if (lane == 0 && grp + gstride < n_groups) { fence_proxy_async(); issue(grp + gstride); }
                 pk::dif_pre<P, XBE>(v, p, tab, t);
             } else {
                 if (MODE == ROW_INIT) {
@@ -173,18 +220,52 @@ __global__ void __launch_bounds__(RowPkCfg<N, XBE>::THREADS, 1) row_pk_kernel(Ro
             pk::dit_post<P, XBE>(p, v, tab, t);
             if (active) {
 #pragma unroll
-                for (int e = 0; e < 64; ++e)
-                    if (in_band(e)) row[t + T * e] = v[e];
+                for (int e = 0; e < 64; ++e) {
+                    if (!in_band(e)) continue;
+                    const int kx = t + T * e;
+                    if (LAYOUT == LAY_NATURAL) { row[kx] = v[e]; continue; }
+                    const int j = (XBE < 32 ? e < XBE : kx < xb) ? kx : kx - (N - 2 * xb);      // compact column
+                    row[(size_t)(j >> 3) * g.ny * 8 + (j & 7)] = v[e];
+                }
             }
         }
     }
 }
 
-template <int N, int MODE, int XBE>
+// 4-D tensor map over the blocked mixed space of a wave batch: dims (fastest first) {16 floats = 8 columns, ny rows,
+// 2 xb / 8 tiles, n_waves}; the box {16, 1, 2 xb / 8, 1} is one compact line.  The driver entry point is fetched at
+// run time (no link-time dependency on libcuda).
+static cudaError_t encode_line_map(const RowArgs& g, CUtensorMap* map)
+{
+    typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                 const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                 CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    static std::atomic<void*> cached{nullptr};
+    void* fn = cached.load(std::memory_order_acquire);
+    if (!fn) {
+        cudaDriverEntryPointQueryResult qres;
+        cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
+        if (e != cudaSuccess) return e;
+        if (!fn || qres != cudaDriverEntryPointSuccess) return cudaErrorNotSupported;
+        cached.store(fn, std::memory_order_release);
+    }
+    const cuuint64_t tiles = (cuuint64_t)(2 * g.xband / 8);
+    const cuuint64_t dims[4] = { 16, (cuuint64_t)g.ny, tiles, (cuuint64_t)g.n_waves };
+    const cuuint64_t strides[3] = { 64, (cuuint64_t)g.ny * 64, (cuuint64_t)g.nx * g.ny * 8 };
+    const cuuint32_t box[4] = { 16, 1, (cuuint32_t)tiles, 1 };
+    const cuuint32_t estr[4] = { 1, 1, 1, 1 };
+    if (tiles > 256) return cudaErrorInvalidValue;
+    const CUresult r = ((EncodeFn)fn)(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, (void*)g.a, dims, strides, box, estr,
+                                      CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                      CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
+}
+
+template <int N, int MODE, int XBE, int LAYOUT>
 static cudaError_t launch_row_pk_x(const RowArgs& g, cudaStream_t stream)
 {
     using C = RowPkCfg<N, XBE>;
-    auto kern = row_pk_kernel<N, MODE, XBE>;
+    auto kern = row_pk_kernel<N, MODE, XBE, LAYOUT>;
     static PerDevice once{};
     if (cudaError_t e = opt_in_smem(kern, C::SMEM, once); e != cudaSuccess) return e;
     const long long n_lines = (long long)g.n_waves * g.ny;
@@ -192,16 +273,29 @@ static cudaError_t launch_row_pk_x(const RowArgs& g, cudaStream_t stream)
     if (n_groups == 0) return cudaSuccess;
     long long grid = (n_groups + C::WARPS - 1) / C::WARPS;
     if (grid > num_sms()) grid = num_sms();
-    return launch_pdl(kern, (unsigned)grid, C::THREADS, C::SMEM, stream, g);
+    CUtensorMap map;
+    std::memset(&map, 0, sizeof(map));
+    if (LAYOUT == LAY_B8_TMA && MODE != ROW_INIT)
+        if (cudaError_t e = encode_line_map(g, &map); e != cudaSuccess) return e;
+    return launch_pdl(kern, (unsigned)grid, C::THREADS, C::SMEM, stream, g, map);
 }
+
+#ifndef PRISM_B8_ROW_LOADER
+#define PRISM_B8_ROW_LOADER LAY_B8_TMA
+#endif
 
 template <int N, int MODE>
 static cudaError_t launch_row_pk_t(const RowArgs& g, cudaStream_t stream)
 {
     constexpr int XB = DefaultBand<N>::XB, T = N / 64;
     static_assert(XB % T == 0, "default band must be a whole number of register slots");
-    if (g.xband == XB) return launch_row_pk_x<N, MODE, XB / T>(g, stream);
-    return launch_row_pk_x<N, MODE, 32>(g, stream);
+    if (g.blocked) {
+        if (g.out == g.a && MODE == ROW_FINAL) return cudaErrorInvalidValue;      // the layouts differ: not in place
+        if (g.xband == XB) return launch_row_pk_x<N, MODE, XB / T, PRISM_B8_ROW_LOADER>(g, stream);
+        return launch_row_pk_x<N, MODE, 32, PRISM_B8_ROW_LOADER>(g, stream);
+    }
+    if (g.xband == XB) return launch_row_pk_x<N, MODE, XB / T, LAY_NATURAL>(g, stream);
+    return launch_row_pk_x<N, MODE, 32, LAY_NATURAL>(g, stream);
 }
 
 template <int N>
@@ -395,6 +489,184 @@ __global__ void __launch_bounds__(ColPkCfg<N>::THREADS, 1) col_pk_kernel(ColArgs
     }
 }
 
+// =============================================================================
+// Column pass on the blocked layout "B8" (top of this file)
+// =============================================================================
+// One team of 8 warps per CTA works on one tile [N rows] x [8 columns] = 128 KB, which is one contiguous run of the
+// blocked layout: a few bulk copies (TMA engine, mbarrier transaction count) land it in shared memory, every thread
+// takes its 64 points into registers, and the landing buffer is refilled with the next tile at once, so the fetch
+// of tile k + 1 overlaps the whole computation of tile k.  The two half-length transforms exchange through a
+// separate 8-byte plane used twice (real parts, then imaginary parts).  Results leave the registers as 8-byte
+// stores of which a warp instruction covers 4 rows x 64 B = 256 contiguous bytes.  The y-factor of the propagator
+// sits in shared memory (with 216 KB of it in use there is next to no L1 left).
+template <int N>
+struct ColB8Cfg {
+    using P = pk::PkPlan<N>;
+    static constexpr int T = P::T;                               // threads per column
+    static constexpr int W = 8;                                  // columns per tile
+    static constexpr int THREADS = W * T;
+    static constexpr int LPW = 32 / W;                           // threads of one column inside a warp
+    static constexpr int TILE_BYTES = N * W * 8;
+    static constexpr int X_BYTES = P::XPAD * W * 8;              // one 8-byte plane, used in two phases
+    static constexpr int TWB = round_up_c(P::TW_BYTES, 128);
+    static constexpr int PYB = N * 8;
+    static constexpr size_t SMEM = PIPE_HEADER + TWB + PYB + (size_t)TILE_BYTES + X_BYTES;
+    static constexpr int CHUNKS = 4;                             // bulk copies per tile
+    static_assert(THREADS == 256 && (THREADS / 32) * LPW == T, "team shape");
+    static_assert(SMEM <= PIPE_SMEM_MAX, "tile + exchange plane do not fit");
+};
+
+template <int N, int MODE, int YBE>
+__global__ void __launch_bounds__(ColB8Cfg<N>::THREADS, 1) col_b8_kernel(ColArgs g)
+{
+    using C = ColB8Cfg<N>;
+    using P = typename C::P;
+    constexpr int T = P::T, W = C::W;
+    constexpr bool LOADS = (MODE != COL_MS_INIT);
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw);
+    float2* tab = reinterpret_cast<float2*>(smem_raw + PIPE_HEADER);
+    float4* py_s = reinterpret_cast<float4*>(smem_raw + PIPE_HEADER + C::TWB);            // pairs (P_y[2j], P_y[2j+1])
+    float2* tile = reinterpret_cast<float2*>(smem_raw + PIPE_HEADER + C::TWB + C::PYB);    // [N][8]
+    float2* xch = reinterpret_cast<float2*>(smem_raw + PIPE_HEADER + C::TWB + C::PYB + C::TILE_BYTES);
+    const int tid = threadIdx.x, lane = tid & 31, c = lane % W, t = (tid >> 5) * C::LPW + lane / W;
+
+    pk::fill_tables<P>(tab, g.tw_y, tid, C::THREADS);
+    if (MODE != COL_MS_INIT)
+        for (int i = tid; i < N; i += C::THREADS) reinterpret_cast<float2*>(py_s)[i] = __ldg(g.prop_y + i);
+    if (LOADS && tid == 0) { mbar_init(full, 1); mbar_fence_init(); }
+    __syncthreads();
+    griddep_wait();                          // the previous kernel of the slice loop has completed (pipe_ptx.cuh)
+    griddep_launch();
+
+    const int xb = g.xband, nx = g.nx;
+    const int tiles_per_wave = 2 * xb / W;
+    const size_t wave_stride = (size_t)N * nx;
+    const long long n_items = (long long)g.n_waves * tiles_per_wave;
+    const long long n_local = (n_items > blockIdx.x) ? (n_items - blockIdx.x + gridDim.x - 1) / gridDim.x : 0;
+    auto locate = [&](long long k, int& w, int& j) {
+        const long long item = blockIdx.x + k * (long long)gridDim.x;
+        w = (int)(item / tiles_per_wave);
+        j = (int)(item % tiles_per_wave);
+    };
+    // thread 0: start the bulk copies of local item k into the landing buffer
+    auto load = [&](long long k) {
+        int w, j;
+        locate(k, w, j);
+        const unsigned char* src = reinterpret_cast<const unsigned char*>(g.a + (size_t)w * wave_stride + (size_t)j * N * W);
+        mbar_expect_tx(full, (unsigned)C::TILE_BYTES);
+#pragma unroll
+        for (int i = 0; i < C::CHUNKS; ++i)
+            bulk_g2s(reinterpret_cast<unsigned char*>(tile) + i * (C::TILE_BYTES / C::CHUNKS),
+                     src + i * (C::TILE_BYTES / C::CHUNKS), (unsigned)(C::TILE_BYTES / C::CHUNKS), full);
+    };
+    if (LOADS && tid == 0 && n_local > 0) load(0);
+    auto sync = [] { __syncthreads(); };
+    const pk::XchgPhase sm{ xch + c, W };
+
+    for (long long k = 0; k < n_local; ++k) {
+        int w, j;
+        locate(k, w, j);
+        const int jc = j * W + c;                                  // compact column
+        const int kxi = jc < xb ? jc : nx - 2 * xb + jc;           // its array slot along kx
+        C2 p[32];
+
+        if (MODE == COL_MS_INIT) {
+            // Psi0(kx, ky) = A_k exp(-i chi_k) exp(-2 pi i (kx xp / lx + ky yp / ly)) at ky = 2 j, 2 j + 1
+            const int pr = g.probe0 + w;
+            const int pxi = pr % g.probes_x, pyi = pr / g.probes_x;
+            const float2 ex = __ldg(g.phase_x + (size_t)pxi * nx + kxi);
+            const float4* ap = reinterpret_cast<const float4*>(g.aperture_t + (size_t)kxi * N);
+            const float4* ey = reinterpret_cast<const float4*>(g.phase_y + (size_t)pyi * N);
+#pragma unroll
+            for (int e = 0; e < 32; ++e) {
+                const int m = t + T * e;
+                const float4 a = __ldg(ap + m), y = __ldg(ey + m);
+                const float2 v0 = cmul(cmul(make_float2(a.x, a.y), ex), make_float2(y.x, y.y));
+                const float2 v1 = cmul(cmul(make_float2(a.z, a.w), ex), make_float2(y.z, y.w));
+                p[e] = { make_float2(v0.y, v1.y), make_float2(v0.x, v1.x) };       // (im, re): inverse = swapped forward
+            }
+        } else {
+            float2 v[64];
+            mbar_wait(full, (unsigned)(k & 1));
+#pragma unroll
+            for (int e = 0; e < 64; ++e) v[e] = tile[(t + T * e) * W + c];
+            // the landing buffer is free once every thread has taken its points: refill it with the next tile
+            __syncthreads();
+            if (tid == 0 && k + 1 < n_local) { fence_proxy_async(); load(k + 1); }
+            pk::dif_pre<P, 32>(v, p, tab, t);
+            pk::fft_half<P>(p, tab, t, sm, sync);
+            // Fresnel propagator with the 2/3 band-limit (Eq. 2; BASELINE.json) at ky = 2 j, 2 j + 1
+            const float2 pxv = __ldg(g.prop_x + kxi);
+            const int lim = __ldg(g.ky_lim + kxi);
+#pragma unroll
+            for (int e = 0; e < 32; ++e) {
+                if (YBE > 0 && e >= YBE && e < 32 - YBE) { p[e] = { make_float2(0.f, 0.f), make_float2(0.f, 0.f) }; continue; }
+                const int m0 = 2 * (t + T * e);
+                const int ky0 = e < 16 ? m0 : N - m0, ky1 = e < 16 ? m0 + 1 : N - m0 - 1;     // |ky|
+                const float4 q = py_s[t + T * e];
+                float2 pr0 = cmul(pxv, make_float2(q.x, q.y)), pr1 = cmul(pxv, make_float2(q.z, q.w));
+                if (ky0 > lim) pr0 = make_float2(0.f, 0.f);
+                if (ky1 > lim) pr1 = make_float2(0.f, 0.f);
+                p[e] = pk::cmul2(p[e], make_float2(pr0.x, pr1.x), make_float2(pr0.y, pr1.y));
+                if (MODE == COL_STEP) p[e] = pk::cswap(p[e]);
+            }
+        }
+
+        if (MODE == COL_STEP || MODE == COL_MS_INIT) {
+            float2 v[64];
+            pk::fft_half<P>(p, tab, t, sm, sync);
+            pk::dit_post<P, 32>(p, v, tab, t);
+            float2* dst = g.a + (size_t)w * wave_stride + (size_t)j * N * W + c;
+#pragma unroll
+            for (int e = 0; e < 64; ++e) dst[(t + T * e) * W] = make_float2(v[e].y, v[e].x);
+        } else {
+            // detector-plane intensity, ky contiguous
+            float2* dst = reinterpret_cast<float2*>(g.intensity + ((size_t)w * nx + kxi) * N);
+#pragma unroll
+            for (int e = 0; e < 32; ++e) {
+                const float2 i2 = pk::fma2(p[e].x, p[e].x, pk::mul2(p[e].y, p[e].y));
+                dst[t + T * e] = make_float2(i2.x * g.scale, i2.y * g.scale);
+            }
+        }
+    }
+}
+
+template <int N, int MODE, int YBE>
+static cudaError_t launch_col_b8_s(const ColArgs& g, cudaStream_t stream)
+{
+    using C = ColB8Cfg<N>;
+    auto kern = col_b8_kernel<N, MODE, YBE>;
+    static PerDevice once{};
+    if (cudaError_t e = opt_in_smem(kern, C::SMEM, once); e != cudaSuccess) return e;
+    if (g.xband % C::W) return cudaErrorInvalidValue;
+    const long long n_items = (long long)g.n_waves * (2 * g.xband / C::W);
+    if (n_items == 0) return cudaSuccess;
+    long long grid = n_items;
+    if (grid > num_sms()) grid = num_sms();
+    return launch_pdl(kern, (unsigned)grid, C::THREADS, C::SMEM, stream, g);
+}
+
+template <int N, int MODE>
+static cudaError_t launch_col_b8_t(const ColArgs& g, cudaStream_t stream)
+{
+    constexpr int YB = DefaultBand<N>::XB, T = N / 64;
+    if (g.yband == YB) return launch_col_b8_s<N, MODE, YB / (2 * T)>(g, stream);
+    return launch_col_b8_s<N, MODE, 0>(g, stream);
+}
+
+static cudaError_t launch_col_b8(ColMode mode, const ColArgs& g, cudaStream_t stream)
+{
+    if (g.ny != 2048) return cudaErrorInvalidValue;
+    switch (mode) {
+        case COL_STEP:     return launch_col_b8_t<2048, COL_STEP>(g, stream);
+        case COL_MS_INIT:  return launch_col_b8_t<2048, COL_MS_INIT>(g, stream);
+        case COL_MS_FINAL: return launch_col_b8_t<2048, COL_MS_FINAL>(g, stream);
+        default: break;
+    }
+    return cudaErrorInvalidValue;
+}
+
 template <int N, int MODE, bool SQ, int YBE>
 static cudaError_t launch_col_pk_s(const ColArgs& g, cudaStream_t stream)
 {
@@ -435,6 +707,7 @@ static cudaError_t launch_col_pk_n(ColMode mode, const ColArgs& g, cudaStream_t 
 cudaError_t launch_col_pk(ColMode mode, const ColArgs& g, cudaStream_t stream)
 {
     if (g.xband < 4 || 2 * g.xband > g.nx) return cudaErrorInvalidValue;
+    if (g.blocked) return launch_col_b8(mode, g, stream);
     switch (g.ny) {
         case 1024: return launch_col_pk_n<1024>(mode, g, stream);
         case 2048: return launch_col_pk_n<2048>(mode, g, stream);
