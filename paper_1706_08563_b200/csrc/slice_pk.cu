@@ -60,18 +60,8 @@ struct RowPkCfg {
     static constexpr size_t SMEM = PIPE_HEADER + TWB + (size_t)WARPS * PER_WARP;
 };
 
-// LAYOUT of mixed space: LAY_NATURAL a[w][y][kx]; LAY_B8_CPA / LAY_B8_TMA blocked "B8" (see the top of this file),
-// the line gathered by 16-byte cp.async copies of all lanes / by one 4-D TMA tensor box {8, 1, 2 xb / 8, 1}.
-enum { LAY_NATURAL = 0, LAY_B8_CPA = 1, LAY_B8_TMA = 2 };
-__device__ __forceinline__ void tensor_g2s_4d(void* smem_dst, const CUtensorMap* map, int c0, int c1, int c2, int c3,
-                                              uint64_t* bar)
-{
-    asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
-                 ::"r"(smem_u32(smem_dst)), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(smem_u32(bar)) : "memory");
-}
-
-template <int N, int MODE, int XBE, int LAYOUT>
-__global__ void __launch_bounds__(RowPkCfg<N, XBE>::THREADS, 1) row_pk_kernel(RowArgs g, const __grid_constant__ CUtensorMap tmap)
+template <int N, int MODE, int XBE>
+__global__ void __launch_bounds__(RowPkCfg<N, XBE>::THREADS, 1) row_pk_kernel(RowArgs g)
 {
     using C = RowPkCfg<N, XBE>;
     using P = typename C::P;
@@ -86,36 +76,18 @@ __global__ void __launch_bounds__(RowPkCfg<N, XBE>::THREADS, 1) row_pk_kernel(Ro
     float2* xch = reinterpret_cast<float2*>(mine + C::LAND_BYTES);             // [LPW][XPAD]
 
     pk::fill_tables<P>(tab, g.tw_x, tid, C::THREADS);
-    if (MODE != ROW_INIT && lane == 0) { mbar_init(&bars[warp], LAYOUT == LAY_B8_CPA ? 32 : 1); mbar_fence_init(); }
+    if (MODE != ROW_INIT && lane == 0) { mbar_init(&bars[warp], 1); mbar_fence_init(); }
     __syncthreads();
     griddep_wait();                          // the previous kernel of the slice loop has completed (pipe_ptx.cuh)
     griddep_launch();
 
-    const size_t wave_stride = (size_t)g.ny * N;
     const long long n_lines = (long long)g.n_waves * g.ny;
     const long long n_groups = (n_lines + LPW - 1) / LPW;
     const long long gw = (long long)blockIdx.x * C::WARPS + warp, gstride = (long long)gridDim.x * C::WARPS;
     const int xb = XBE < 32 ? XBE * T : g.xband;                 // in-band columns: [0, xb) and [N - xb, N)
 
-    // start the copies of line group `grp` into the landing buffer (compact: [0, xb) then [N - xb, N)).
-    // LAY_B8_CPA: called by every lane of the warp; otherwise by lane 0 only.
+    // lane 0: start the bulk copies of line group `grp` into the landing buffer
     auto issue = [&](long long grp) {
-        if (LAYOUT == LAY_B8_CPA) {
-#pragma unroll
-            for (int l = 0; l < LPW; ++l) {
-                const long long line = grp * LPW + l;
-                if (line < n_lines) {
-                    const int y = (int)(line / g.n_waves), w = (int)(line % g.n_waves);
-                    const float2* src = g.a + (size_t)w * wave_stride + (size_t)y * 8;
-                    float2* dst = land + l * C::LANDW;
-                    // 16-byte chunk q of the compact line: piece q / 4 (64 bytes of tile q / 4), quarter q % 4
-                    for (int q = lane; q < xb; q += 32)
-                        cp_async16(dst + 2 * q, src + (size_t)(q >> 2) * g.ny * 8 + 2 * (q & 3));
-                }
-            }
-            cp_async_arrive(&bars[warp]);
-            return;
-        }
         int n_act = 0;
 #pragma unroll
         for (int l = 0; l < LPW; ++l) n_act += (grp * LPW + l < n_lines);
@@ -125,18 +97,14 @@ __global__ void __launch_bounds__(RowPkCfg<N, XBE>::THREADS, 1) row_pk_kernel(Ro
             const long long line = grp * LPW + l;
             if (line < n_lines) {
                 const int y = (int)(line / g.n_waves), w = (int)(line % g.n_waves);
+                const float2* row = g.a + ((size_t)w * g.ny + y) * N;
                 float2* dst = land + l * C::LANDW;
-                if (LAYOUT == LAY_B8_TMA) {
-                    tensor_g2s_4d(dst, &tmap, 0, y, 0, w, &bars[warp]);
-                } else {
-                    const float2* row = g.a + ((size_t)w * g.ny + y) * N;
-                    bulk_g2s(dst, row, (unsigned)(xb * sizeof(float2)), &bars[warp]);
-                    bulk_g2s(dst + xb, row + (N - xb), (unsigned)(xb * sizeof(float2)), &bars[warp]);
-                }
+                bulk_g2s(dst, row, (unsigned)(xb * sizeof(float2)), &bars[warp]);
+                bulk_g2s(dst + xb, row + (N - xb), (unsigned)(xb * sizeof(float2)), &bars[warp]);
             }
         }
     };
-    if (MODE != ROW_INIT && (LAYOUT == LAY_B8_CPA || lane == 0) && gw < n_groups) issue(gw);
+    if (MODE != ROW_INIT && lane == 0 && gw < n_groups) issue(gw);
 
     const pk::XchgPhase sm{ xch + ll * P::XPAD, 1 };
     auto sync = [] { __syncwarp(); };
@@ -148,8 +116,7 @@ __global__ void __launch_bounds__(RowPkCfg<N, XBE>::THREADS, 1) row_pk_kernel(Ro
         const bool active = line < n_lines;
         if (!active) line = n_lines - 1;                 // keep every lane in the warp barriers
         const int y = (int)(line / g.n_waves), w = (int)(line % g.n_waves);
-        // natural: the row itself; blocked: row y of tile 0 of the wave (column j lives (j >> 3) ny 8 + (j & 7) further on)
-        float2* row = LAYOUT == LAY_NATURAL ? g.a + ((size_t)w * g.ny + y) * N : g.a + (size_t)w * wave_stride + (size_t)y * 8;
+        float2* row = g.a + ((size_t)w * g.ny + y) * N;
         C2 p[32];
 
         // Phase 0 builds the pairs the first half-length transform runs on (plane wave, or the landed line after
@@ -174,8 +141,7 @@ __global__ void __launch_bounds__(RowPkCfg<N, XBE>::THREADS, 1) row_pk_kernel(Ro
                 }
                 // the landing buffer is free once every lane has read its points
                 __syncwarp();
-                if (LAYOUT == LAY_B8_CPA) { if (grp + gstride < n_groups) issue(grp + gstride); }
-                else if (lane == 0 && grp + gstride < n_groups) { fence_proxy_async(); issue(grp + gstride); }
+                if (lane == 0 && grp + gstride < n_groups) { fence_proxy_async(); issue(grp + gstride); }
                 pk::dif_pre<P, XBE>(v, p, tab, t);
             } else {
                 if (MODE == ROW_INIT) {
@@ -220,12 +186,255 @@ __global__ void __launch_bounds__(RowPkCfg<N, XBE>::THREADS, 1) row_pk_kernel(Ro
             pk::dit_post<P, XBE>(p, v, tab, t);
             if (active) {
 #pragma unroll
-                for (int e = 0; e < 64; ++e) {
-                    if (!in_band(e)) continue;
-                    const int kx = t + T * e;
-                    if (LAYOUT == LAY_NATURAL) { row[kx] = v[e]; continue; }
-                    const int j = (XBE < 32 ? e < XBE : kx < xb) ? kx : kx - (N - 2 * xb);      // compact column
-                    row[(size_t)(j >> 3) * g.ny * 8 + (j & 7)] = v[e];
+                for (int e = 0; e < 64; ++e)
+                    if (in_band(e)) row[t + T * e] = v[e];
+            }
+        }
+    }
+}
+
+template <int N, int MODE, int XBE>
+static cudaError_t launch_row_pk_x(const RowArgs& g, cudaStream_t stream)
+{
+    using C = RowPkCfg<N, XBE>;
+    auto kern = row_pk_kernel<N, MODE, XBE>;
+    static PerDevice once{};
+    if (cudaError_t e = opt_in_smem(kern, C::SMEM, once); e != cudaSuccess) return e;
+    const long long n_lines = (long long)g.n_waves * g.ny;
+    const long long n_groups = (n_lines + C::LPW - 1) / C::LPW;
+    if (n_groups == 0) return cudaSuccess;
+    long long grid = (n_groups + C::WARPS - 1) / C::WARPS;
+    if (grid > num_sms()) grid = num_sms();
+    return launch_pdl(kern, (unsigned)grid, C::THREADS, C::SMEM, stream, g);
+}
+
+template <int N, int MODE>
+static cudaError_t launch_row_pk_t(const RowArgs& g, cudaStream_t stream)
+{
+    constexpr int XB = DefaultBand<N>::XB, T = N / 64;
+    static_assert(XB % T == 0, "default band must be a whole number of register slots");
+    if (g.xband == XB) return launch_row_pk_x<N, MODE, XB / T>(g, stream);
+    return launch_row_pk_x<N, MODE, 32>(g, stream);
+}
+
+template <int N>
+static cudaError_t launch_row_pk_n(RowMode mode, const RowArgs& g, cudaStream_t stream)
+{
+    switch (mode) {
+        case ROW_INIT:  return launch_row_pk_t<N, ROW_INIT>(g, stream);
+        case ROW_STEP:  return launch_row_pk_t<N, ROW_STEP>(g, stream);
+        case ROW_FINAL: return launch_row_pk_t<N, ROW_FINAL>(g, stream);
+        default: break;
+    }
+    return cudaErrorInvalidValue;
+}
+
+template <int N> static cudaError_t launch_row_b8(RowMode mode, const RowArgs& g, cudaStream_t stream);   // below
+
+cudaError_t launch_row_pk(RowMode mode, const RowArgs& g, cudaStream_t stream)
+{
+    if (g.xband < 32 || g.xband % 32 || 2 * g.xband > g.nx) return cudaErrorInvalidValue;
+    if (g.blocked) return g.nx == 2048 ? launch_row_b8<2048>(mode, g, stream) : cudaErrorInvalidValue;
+    switch (g.nx) {
+        case 1024: return launch_row_pk_n<1024>(mode, g, stream);
+        case 2048: return launch_row_pk_n<2048>(mode, g, stream);
+    }
+    return cudaErrorInvalidValue;
+}
+
+// =============================================================================
+// Row pass on the blocked layout "B8" (top of this file)
+// =============================================================================
+// A line of blocked mixed space is 2 xb / 8 pieces of 64 bytes, 128 KB apart; pieces of consecutive rows y are
+// adjacent.  So that the DRAM sees runs and not isolated 64-byte pieces, lines are ordered by (block of G rows,
+// group of 8 waves): CTA b of the G resident CTAs owns row y = yb G + b of the current row block and its 8 warps
+// take 8 different waves of that row -- at any moment the grid reads and writes G consecutive rows of a few waves,
+// i.e. runs of G x 64 B per tile.  Every warp of a CTA then needs the same row of the transmission function for
+// n_waves / 8 lines in a row: it is brought into shared memory once per row block (one bulk copy), which takes the
+// t_s loads out of the L1 / long-scoreboard path.
+// LOADER: the line is gathered by one 4-D TMA tensor box {8 columns, 1 row, 2 xb / 8 tiles, 1 wave} issued by one
+// lane (LAY_B8_TMA), or by 16-byte cp.async copies of all lanes (LAY_B8_CPA).
+enum { LAY_B8_CPA = 1, LAY_B8_TMA = 2 };
+__device__ __forceinline__ void tensor_g2s_4d(void* smem_dst, const CUtensorMap* map, int c0, int c1, int c2, int c3,
+                                              uint64_t* bar)
+{
+    asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
+                 ::"r"(smem_u32(smem_dst)), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(smem_u32(bar)) : "memory");
+}
+
+template <int N, int XBE>
+struct RowB8Cfg {
+    using P = pk::PkPlan<N>;
+    using B = RowPkCfg<N, XBE>;
+    static constexpr int T = P::T, LPW = 32 / T;
+    static constexpr int LANDW = B::LANDW, LAND_BYTES = B::LAND_BYTES, PER_WARP = B::PER_WARP, TWB = B::TWB;
+    static constexpr int T_BYTES = N * 8;                          // one row of the transmission function
+    static constexpr int BY_SMEM = (PIPE_SMEM_MAX - PIPE_HEADER - TWB - T_BYTES) / PER_WARP;
+    static constexpr int WARPS = BY_SMEM < PK_ROW_MAX_WARPS ? BY_SMEM : PK_ROW_MAX_WARPS;
+    static constexpr int THREADS = WARPS * 32;
+    static constexpr size_t SMEM = PIPE_HEADER + TWB + T_BYTES + (size_t)WARPS * PER_WARP;
+};
+
+template <int N, int MODE, int XBE, int LOADER>
+__global__ void __launch_bounds__(RowB8Cfg<N, XBE>::THREADS, 1) row_b8_kernel(RowArgs g, const __grid_constant__ CUtensorMap tmap)
+{
+    using C = RowB8Cfg<N, XBE>;
+    using P = typename C::P;
+    constexpr int T = P::T, LPW = C::LPW, WARPS = C::WARPS;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw);                    // [WARPS] landing buffers, [WARPS] t row
+    float2* tab = reinterpret_cast<float2*>(smem_raw + PIPE_HEADER);
+    const float4* trow = reinterpret_cast<const float4*>(smem_raw + PIPE_HEADER + C::TWB);
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int ll = lane / T, t = lane % T;
+    unsigned char* mine = smem_raw + PIPE_HEADER + C::TWB + C::T_BYTES + (size_t)warp * C::PER_WARP;
+    float2* land = reinterpret_cast<float2*>(mine);                            // [LPW][LANDW]
+    float2* xch = reinterpret_cast<float2*>(mine + C::LAND_BYTES);             // [LPW][XPAD]
+    uint64_t* tbar = &bars[WARPS];
+
+    pk::fill_tables<P>(tab, g.tw_x, tid, C::THREADS);
+    if (lane == 0) {
+        if (MODE != ROW_INIT) mbar_init(&bars[warp], LOADER == LAY_B8_CPA ? 32 : 1);
+        if (warp == 0) mbar_init(tbar, 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+    griddep_wait();                          // the previous kernel of the slice loop has completed (pipe_ptx.cuh)
+    griddep_launch();
+
+    const int G = gridDim.x, bid = blockIdx.x;
+    const size_t wave_stride = (size_t)g.ny * N;
+    const int xb = XBE < 32 ? XBE * T : g.xband;                 // in-band columns: [0, xb) and [N - xb, N)
+    // this warp's lines: rows y = yb G + bid (yb < my_yblocks), wave groups wg < my_wgroups with waves
+    // (wg WARPS + warp) LPW + l; `seq` = yb my_wgroups + wg numbers them in processing order
+    const int my_yblocks = bid < g.ny ? (g.ny - bid + G - 1) / G : 0;
+    const int first_wave = warp * LPW;
+    const int my_wgroups = first_wave < g.n_waves ? (g.n_waves - first_wave + WARPS * LPW - 1) / (WARPS * LPW) : 0;
+    const long long my_lines = (long long)my_yblocks * my_wgroups;
+
+    // start the copies of line group `seq` into the landing buffer (compact: [0, xb) then [N - xb, N)).
+    // LAY_B8_CPA: called by every lane of the warp; LAY_B8_TMA: by lane 0.
+    auto issue = [&](long long seq) {
+        const int y = (int)(seq / my_wgroups) * G + bid, w0 = ((int)(seq % my_wgroups) * WARPS + warp) * LPW;
+        if (LOADER == LAY_B8_CPA) {
+#pragma unroll
+            for (int l = 0; l < LPW; ++l) {
+                if (w0 + l < g.n_waves) {
+                    const float2* src = g.a + (size_t)(w0 + l) * wave_stride + (size_t)y * 8;
+                    float2* dst = land + l * C::LANDW;
+                    // 16-byte chunk q of the compact line: quarter q % 4 of the 64-byte piece in tile q / 4
+                    for (int q = lane; q < xb; q += 32)
+                        cp_async16(dst + 2 * q, src + (size_t)(q >> 2) * g.ny * 8 + 2 * (q & 3));
+                }
+            }
+            cp_async_arrive(&bars[warp]);
+        } else {
+            int n_act = 0;
+#pragma unroll
+            for (int l = 0; l < LPW; ++l) n_act += (w0 + l < g.n_waves);
+            mbar_expect_tx(&bars[warp], (unsigned)(n_act * 2 * xb * (int)sizeof(float2)));
+#pragma unroll
+            for (int l = 0; l < LPW; ++l)
+                if (w0 + l < g.n_waves) tensor_g2s_4d(land + l * C::LANDW, &tmap, 0, y, 0, w0 + l, &bars[warp]);
+        }
+    };
+    if (MODE != ROW_INIT && (LOADER == LAY_B8_CPA || lane == 0) && my_lines > 0) issue(0);
+
+    const pk::XchgPhase sm{ xch + ll * P::XPAD, 1 };
+    auto sync = [] { __syncwarp(); };
+    auto in_band = [&](int e) { return XBE < 32 ? pk::kept<XBE>(e) : (t + T * e < xb || t + T * e >= N - xb); };
+
+    long long seq = 0;
+    for (int yb = 0; yb < my_yblocks; ++yb) {
+        const int y = yb * G + bid;
+        if (MODE != ROW_FINAL) {
+            // the row of t_s every warp of this CTA multiplies by until the next row block
+            __syncthreads();                             // every warp is done with the previous row
+            if (tid == 0) {
+                fence_proxy_async();
+                mbar_expect_tx(tbar, (unsigned)C::T_BYTES);
+                bulk_g2s(const_cast<float4*>(trow), g.t + (size_t)y * N, (unsigned)C::T_BYTES, tbar);
+            }
+            mbar_wait(tbar, (unsigned)(yb & 1));
+        }
+        for (int wg = 0; wg < my_wgroups; ++wg, ++seq) {
+            int w = (wg * WARPS + warp) * LPW + ll;
+            const bool active = w < g.n_waves;
+            if (!active) w = g.n_waves - 1;                  // keep every lane in the warp barriers
+            // row y of tile 0 of the wave; column j of the compact band lives (j >> 3) ny 8 + (j & 7) further on
+            float2* row = g.a + (size_t)w * wave_stride + (size_t)y * 8;
+            C2 p[32];
+
+            constexpr int PH0 = (MODE == ROW_INIT) ? 1 : 0, PH1 = (MODE == ROW_FINAL) ? 1 : 2;
+#pragma unroll 1
+            for (int ph = PH0; ph < PH1; ++ph) {
+                if (ph == 0) {
+                    float2 v[64];
+                    mbar_wait(&bars[warp], (unsigned)(seq & 1));
+                    const float2* lbase = land + ll * C::LANDW;
+#pragma unroll
+                    for (int e = 0; e < 64; ++e) {
+                        const int kx = t + T * e;
+                        int pos;                                    // compact landing: [0, xb) then [N - xb, N)
+                        if (XBE < 32) pos = e < XBE ? kx : kx - (N - 2 * xb);
+                        else pos = kx < xb ? kx : (kx >= N - xb ? kx - (N - 2 * xb) : 0);
+                        if (XBE < 32 && !pk::kept<XBE>(e)) { v[e] = make_float2(0.f, 0.f); continue; }
+                        const float2 q = lbase[pos];
+                        v[e] = in_band(e) ? make_float2(q.y, q.x) : make_float2(0.f, 0.f);   // (im, re): inverse = swapped forward
+                    }
+                    // the landing buffer is free once every lane has read its points
+                    __syncwarp();
+                    if (seq + 1 < my_lines) {
+                        if (LOADER == LAY_B8_CPA) issue(seq + 1);
+                        else if (lane == 0) { fence_proxy_async(); issue(seq + 1); }
+                    }
+                    pk::dif_pre<P, XBE>(v, p, tab, t);
+                } else {
+                    if (MODE == ROW_INIT) {
+                        // plane wave exp(+2 pi i (kx x / nx + ky y / ny)) * amplitude at x = 2 j, 2 j + 1
+                        const int2 b = g.beams[w];
+                        const float2 wy = __ldg(g.tw_y + ((b.y * y) & (g.ny - 1)));
+                        const float2 base = make_float2(wy.x * g.scale, -wy.y * g.scale);
+                        const float2 b0 = cmul_conj(base, __ldg(g.tw_x + ((b.x * (2 * t)) & (N - 1))));
+                        const float2 b1 = cmul_conj(base, __ldg(g.tw_x + ((b.x * (2 * t + 1)) & (N - 1))));
+#pragma unroll
+                        for (int e = 0; e < 32; ++e) {
+                            const float2 we = __ldg(g.tw_x + ((b.x * (2 * T * e)) & (N - 1)));
+                            const float2 v0 = cmul_conj(b0, we), v1 = cmul_conj(b1, we);
+                            p[e] = { make_float2(v0.x, v1.x), make_float2(v0.y, v1.y) };
+                        }
+                    } else {
+#pragma unroll
+                        for (int e = 0; e < 32; ++e) p[e] = pk::cswap(p[e]);       // back from the swapped inverse
+                    }
+                    // transmission function in pair layout: (re(2j), re(2j+1), im(2j), im(2j+1))
+#pragma unroll
+                    for (int e = 0; e < 32; ++e) {
+                        const float4 q = trow[t + T * e];
+                        p[e] = pk::cmul2(p[e], make_float2(q.x, q.y), make_float2(q.z, q.w));
+                    }
+                }
+                pk::fft_half<P>(p, tab, t, sm, sync);
+            }
+
+            if (MODE == ROW_FINAL) {
+                float4* dst = reinterpret_cast<float4*>(g.out + ((size_t)w * g.ny + y) * N);
+                if (active) {
+#pragma unroll
+                    for (int e = 0; e < 32; ++e)       // p holds the swapped inverse: (y, x) are (re, im)
+                        dst[t + T * e] = make_float4(p[e].y.x * g.scale, p[e].x.x * g.scale, p[e].y.y * g.scale, p[e].x.y * g.scale);
+                }
+            } else {
+                float2 v[64];
+                pk::dit_post<P, XBE>(p, v, tab, t);
+                if (active) {
+#pragma unroll
+                    for (int e = 0; e < 64; ++e) {
+                        if (!in_band(e)) continue;
+                        const int kx = t + T * e;
+                        const int j = (XBE < 32 ? e < XBE : kx < xb) ? kx : kx - (N - 2 * xb);      // compact column
+                        row[(size_t)(j >> 3) * g.ny * 8 + (j & 7)] = v[e];
+                    }
                 }
             }
         }
@@ -250,72 +459,49 @@ static cudaError_t encode_line_map(const RowArgs& g, CUtensorMap* map)
         cached.store(fn, std::memory_order_release);
     }
     const cuuint64_t tiles = (cuuint64_t)(2 * g.xband / 8);
+    if (tiles > 256) return cudaErrorInvalidValue;
     const cuuint64_t dims[4] = { 16, (cuuint64_t)g.ny, tiles, (cuuint64_t)g.n_waves };
     const cuuint64_t strides[3] = { 64, (cuuint64_t)g.ny * 64, (cuuint64_t)g.nx * g.ny * 8 };
     const cuuint32_t box[4] = { 16, 1, (cuuint32_t)tiles, 1 };
     const cuuint32_t estr[4] = { 1, 1, 1, 1 };
-    if (tiles > 256) return cudaErrorInvalidValue;
     const CUresult r = ((EncodeFn)fn)(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4, (void*)g.a, dims, strides, box, estr,
                                       CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
                                       CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
 }
 
-template <int N, int MODE, int XBE, int LAYOUT>
-static cudaError_t launch_row_pk_x(const RowArgs& g, cudaStream_t stream)
-{
-    using C = RowPkCfg<N, XBE>;
-    auto kern = row_pk_kernel<N, MODE, XBE, LAYOUT>;
-    static PerDevice once{};
-    if (cudaError_t e = opt_in_smem(kern, C::SMEM, once); e != cudaSuccess) return e;
-    const long long n_lines = (long long)g.n_waves * g.ny;
-    const long long n_groups = (n_lines + C::LPW - 1) / C::LPW;
-    if (n_groups == 0) return cudaSuccess;
-    long long grid = (n_groups + C::WARPS - 1) / C::WARPS;
-    if (grid > num_sms()) grid = num_sms();
-    CUtensorMap map;
-    std::memset(&map, 0, sizeof(map));
-    if (LAYOUT == LAY_B8_TMA && MODE != ROW_INIT)
-        if (cudaError_t e = encode_line_map(g, &map); e != cudaSuccess) return e;
-    return launch_pdl(kern, (unsigned)grid, C::THREADS, C::SMEM, stream, g, map);
-}
-
 #ifndef PRISM_B8_ROW_LOADER
 #define PRISM_B8_ROW_LOADER LAY_B8_TMA
 #endif
 
-template <int N, int MODE>
-static cudaError_t launch_row_pk_t(const RowArgs& g, cudaStream_t stream)
+template <int N, int MODE, int XBE>
+static cudaError_t launch_row_b8_x(const RowArgs& g, cudaStream_t stream)
 {
-    constexpr int XB = DefaultBand<N>::XB, T = N / 64;
-    static_assert(XB % T == 0, "default band must be a whole number of register slots");
-    if (g.blocked) {
-        if (g.out == g.a && MODE == ROW_FINAL) return cudaErrorInvalidValue;      // the layouts differ: not in place
-        if (g.xband == XB) return launch_row_pk_x<N, MODE, XB / T, PRISM_B8_ROW_LOADER>(g, stream);
-        return launch_row_pk_x<N, MODE, 32, PRISM_B8_ROW_LOADER>(g, stream);
-    }
-    if (g.xband == XB) return launch_row_pk_x<N, MODE, XB / T, LAY_NATURAL>(g, stream);
-    return launch_row_pk_x<N, MODE, 32, LAY_NATURAL>(g, stream);
+    using C = RowB8Cfg<N, XBE>;
+    auto kern = row_b8_kernel<N, MODE, XBE, PRISM_B8_ROW_LOADER>;
+    static PerDevice once{};
+    if (cudaError_t e = opt_in_smem(kern, C::SMEM, once); e != cudaSuccess) return e;
+    if (g.n_waves <= 0) return cudaSuccess;
+    if (MODE == ROW_FINAL && g.out == g.a) return cudaErrorInvalidValue;          // the layouts differ: not in place
+    int grid = num_sms();
+    if (grid > g.ny) grid = g.ny;
+    CUtensorMap map;
+    std::memset(&map, 0, sizeof(map));
+    if (PRISM_B8_ROW_LOADER == LAY_B8_TMA && MODE != ROW_INIT)
+        if (cudaError_t e = encode_line_map(g, &map); e != cudaSuccess) return e;
+    return launch_pdl(kern, (unsigned)grid, C::THREADS, C::SMEM, stream, g, map);
 }
 
 template <int N>
-static cudaError_t launch_row_pk_n(RowMode mode, const RowArgs& g, cudaStream_t stream)
+static cudaError_t launch_row_b8(RowMode mode, const RowArgs& g, cudaStream_t stream)
 {
+    constexpr int XB = DefaultBand<N>::XB, T = N / 64;
+    const bool def = g.xband == XB;
     switch (mode) {
-        case ROW_INIT:  return launch_row_pk_t<N, ROW_INIT>(g, stream);
-        case ROW_STEP:  return launch_row_pk_t<N, ROW_STEP>(g, stream);
-        case ROW_FINAL: return launch_row_pk_t<N, ROW_FINAL>(g, stream);
+        case ROW_INIT:  return def ? launch_row_b8_x<N, ROW_INIT, XB / T>(g, stream) : launch_row_b8_x<N, ROW_INIT, 32>(g, stream);
+        case ROW_STEP:  return def ? launch_row_b8_x<N, ROW_STEP, XB / T>(g, stream) : launch_row_b8_x<N, ROW_STEP, 32>(g, stream);
+        case ROW_FINAL: return def ? launch_row_b8_x<N, ROW_FINAL, XB / T>(g, stream) : launch_row_b8_x<N, ROW_FINAL, 32>(g, stream);
         default: break;
-    }
-    return cudaErrorInvalidValue;
-}
-
-cudaError_t launch_row_pk(RowMode mode, const RowArgs& g, cudaStream_t stream)
-{
-    if (g.xband < 32 || g.xband % 32 || 2 * g.xband > g.nx) return cudaErrorInvalidValue;
-    switch (g.nx) {
-        case 1024: return launch_row_pk_n<1024>(mode, g, stream);
-        case 2048: return launch_row_pk_n<2048>(mode, g, stream);
     }
     return cudaErrorInvalidValue;
 }
