@@ -226,11 +226,12 @@ struct XchgPhase {
 // Forward half-length transforms of both lanes: p[e] holds element t + T e (layout in = layout out).
 // SYNC() is a barrier among (at least) the threads of the line; the function begins with one, so the
 // exchange space may alias storage those threads have just read.
-template <class P, class SM, class SYNC>
+// LEAD_SYNC = false: the caller guarantees that barrier already (nothing has touched the exchange space since).
+template <class P, bool LEAD_SYNC = true, class SM, class SYNC>
 __device__ __forceinline__ void fft_half(C2 (&p)[32], const float2* __restrict__ t2, int t, const SM& sm, SYNC sync)
 {
     constexpr int T = P::T;
-    sync();
+    if (LEAD_SYNC) sync();
     Dft<32>::run(p);
     if constexpr (SM::TWO_PHASE) {
 #pragma unroll

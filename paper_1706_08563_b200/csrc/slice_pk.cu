@@ -254,6 +254,9 @@ cudaError_t launch_row_pk(RowMode mode, const RowArgs& g, cudaStream_t stream)
 // t_s loads out of the L1 / long-scoreboard path.
 // LOADER: the line is gathered by one 4-D TMA tensor box {8 columns, 1 row, 2 xb / 8 tiles, 1 wave} issued by one
 // lane (LAY_B8_TMA), or by 16-byte cp.async copies of all lanes (LAY_B8_CPA).
+#ifndef PRISM_B8_ROW_UNROLL_PH
+#define PRISM_B8_ROW_UNROLL_PH 0
+#endif
 enum { LAY_B8_CPA = 1, LAY_B8_TMA = 2 };
 __device__ __forceinline__ void tensor_g2s_4d(void* smem_dst, const CUtensorMap* map, int c0, int c1, int c2, int c3,
                                               uint64_t* bar)
@@ -366,7 +369,11 @@ __global__ void __launch_bounds__(RowB8Cfg<N, XBE>::THREADS, 1) row_b8_kernel(Ro
             C2 p[32];
 
             constexpr int PH0 = (MODE == ROW_INIT) ? 1 : 0, PH1 = (MODE == ROW_FINAL) ? 1 : 2;
+#if PRISM_B8_ROW_UNROLL_PH
+#pragma unroll
+#else
 #pragma unroll 1
+#endif
             for (int ph = PH0; ph < PH1; ++ph) {
                 if (ph == 0) {
                     float2 v[64];
@@ -678,28 +685,31 @@ __global__ void __launch_bounds__(ColPkCfg<N>::THREADS, 1) col_pk_kernel(ColArgs
 // =============================================================================
 // Column pass on the blocked layout "B8" (top of this file)
 // =============================================================================
-// One team of 8 warps per CTA works on one tile [N rows] x [8 columns] = 128 KB, which is one contiguous run of the
-// blocked layout: a few bulk copies (TMA engine, mbarrier transaction count) land it in shared memory, every thread
-// takes its 64 points into registers, and the landing buffer is refilled with the next tile at once, so the fetch
-// of tile k + 1 overlaps the whole computation of tile k.  The two half-length transforms exchange through a
-// separate 8-byte plane used twice (real parts, then imaginary parts).  Results leave the registers as 8-byte
-// stores of which a warp instruction covers 4 rows x 64 B = 256 contiguous bytes.  The y-factor of the propagator
-// sits in shared memory (with 216 KB of it in use there is next to no L1 left).
+// A CTA of 8 warps works on one tile [N rows] x [8 columns] = 128 KB, which is one contiguous run of the blocked
+// layout: a few bulk copies (TMA engine, mbarrier transaction count) land it in shared memory, every thread takes
+// its 64 points into registers, and the landing buffer is refilled with the next tile at once, so the fetch of
+// tile k + 1 overlaps the computation of tile k.  The half-length transforms exchange through a separate 8-byte
+// plane used twice (real parts, then imaginary parts).  The y-factor of the propagator sits in shared memory (with
+// 216 KB of it in use there is next to no L1 left).
+// One team of 256 threads owns all 8 columns, so a warp's store instruction covers 4 rows x 64 B = 256 contiguous
+// bytes.  (Two teams of 128 threads on columns 0-3 / 4-7 of the same tile, skewed by half a tile so that one
+// team's butterflies overlap the other's exchanges, measured slower: 14.6 ms against 13.9 ms per launch -- their
+// stores are 32-byte row segments again and their landing reads conflict two-way.)
+
 template <int N>
 struct ColB8Cfg {
     using P = pk::PkPlan<N>;
     static constexpr int T = P::T;                               // threads per column
     static constexpr int W = 8;                                  // columns per tile
     static constexpr int THREADS = W * T;
-    static constexpr int LPW = 32 / W;                           // threads of one column inside a warp
     static constexpr int TILE_BYTES = N * W * 8;
-    static constexpr int X_BYTES = P::XPAD * W * 8;              // one 8-byte plane, used in two phases
+    static constexpr int X_BYTES = P::XPAD * W * 8;              // 8-byte exchange planes of all columns, used in two phases
     static constexpr int TWB = round_up_c(P::TW_BYTES, 128);
     static constexpr int PYB = N * 8;
     static constexpr size_t SMEM = PIPE_HEADER + TWB + PYB + (size_t)TILE_BYTES + X_BYTES;
     static constexpr int CHUNKS = 4;                             // bulk copies per tile
-    static_assert(THREADS == 256 && (THREADS / 32) * LPW == T, "team shape");
-    static_assert(SMEM <= PIPE_SMEM_MAX, "tile + exchange plane do not fit");
+    static_assert(THREADS == 256, "team shape");
+    static_assert(SMEM <= PIPE_SMEM_MAX, "tile + exchange planes do not fit");
 };
 
 template <int N, int MODE, int YBE>
@@ -708,6 +718,8 @@ __global__ void __launch_bounds__(ColB8Cfg<N>::THREADS, 1) col_b8_kernel(ColArgs
     using C = ColB8Cfg<N>;
     using P = typename C::P;
     constexpr int T = P::T, W = C::W;
+    constexpr int LPW = 32 / W;                                   // threads of one column inside a warp
+    static_assert((C::THREADS / 32) * LPW == T, "team shape");
     constexpr bool LOADS = (MODE != COL_MS_INIT);
     extern __shared__ __align__(128) unsigned char smem_raw[];
     uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw);
@@ -715,7 +727,8 @@ __global__ void __launch_bounds__(ColB8Cfg<N>::THREADS, 1) col_b8_kernel(ColArgs
     float4* py_s = reinterpret_cast<float4*>(smem_raw + PIPE_HEADER + C::TWB);            // pairs (P_y[2j], P_y[2j+1])
     float2* tile = reinterpret_cast<float2*>(smem_raw + PIPE_HEADER + C::TWB + C::PYB);    // [N][8]
     float2* xch = reinterpret_cast<float2*>(smem_raw + PIPE_HEADER + C::TWB + C::PYB + C::TILE_BYTES);
-    const int tid = threadIdx.x, lane = tid & 31, c = lane % W, t = (tid >> 5) * C::LPW + lane / W;
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int c = lane % W, t = (tid >> 5) * LPW + lane / W;
 
     pk::fill_tables<P>(tab, g.tw_y, tid, C::THREADS);
     if (MODE != COL_MS_INIT)
@@ -735,7 +748,7 @@ __global__ void __launch_bounds__(ColB8Cfg<N>::THREADS, 1) col_b8_kernel(ColArgs
         w = (int)(item / tiles_per_wave);
         j = (int)(item % tiles_per_wave);
     };
-    // thread 0: start the bulk copies of local item k into the landing buffer
+    // one thread: start the bulk copies of local item k into the landing buffer
     auto load = [&](long long k) {
         int w, j;
         locate(k, w, j);
@@ -774,17 +787,18 @@ __global__ void __launch_bounds__(ColB8Cfg<N>::THREADS, 1) col_b8_kernel(ColArgs
             }
         } else {
             float2 v[64];
+            // per-column propagator factor and band limit: requested now, used between the transforms
+            const float2 pxv = __ldg(g.prop_x + kxi);
+            const int lim = __ldg(g.ky_lim + kxi);
             mbar_wait(full, (unsigned)(k & 1));
 #pragma unroll
             for (int e = 0; e < 64; ++e) v[e] = tile[(t + T * e) * W + c];
             // the landing buffer is free once every thread has taken its points: refill it with the next tile
-            __syncthreads();
+            sync();
             if (tid == 0 && k + 1 < n_local) { fence_proxy_async(); load(k + 1); }
             pk::dif_pre<P, 32>(v, p, tab, t);
-            pk::fft_half<P>(p, tab, t, sm, sync);
+            pk::fft_half<P, false>(p, tab, t, sm, sync);        // the barrier after the landing reads covers the exchange plane
             // Fresnel propagator with the 2/3 band-limit (Eq. 2; BASELINE.json) at ky = 2 j, 2 j + 1
-            const float2 pxv = __ldg(g.prop_x + kxi);
-            const int lim = __ldg(g.ky_lim + kxi);
 #pragma unroll
             for (int e = 0; e < 32; ++e) {
                 if (YBE > 0 && e >= YBE && e < 32 - YBE) { p[e] = { make_float2(0.f, 0.f), make_float2(0.f, 0.f) }; continue; }
