@@ -460,22 +460,25 @@ def run_prism(name, steps, warmup, world, rank, local, dist, want_cpu_baseline):
     # the nx only (c = prism_band_columns; whole waves below 256 points), real space in full
     band = 2.0 * prism.band_columns(p) / w.nx if min(w.nx, w.ny) >= 256 else 1.0
     mixed, real = 8 * npix * n_beams * band, 8 * npix * n_beams
-    per_launch_bytes = {"row_step": 2 * mixed, "col_step": 2 * mixed, "row_init": mixed, "row_final": mixed + real}
+    # algorithmic bytes per step and kernel class (a class may be split over several launches: the blocked layout runs
+    # ROW_FINAL a few waves at a time)
+    per_step_bytes = {"row_step": 2 * mixed * (w.n_slices - 1), "col_step": 2 * mixed * w.n_slices, "row_init": mixed,
+                      "row_final": mixed + real}
     kernels = {}
     for kname, (ms, cnt) in kern.items():
         entry = {"ms_per_step": ms / inst_steps, "launches_per_step": cnt / inst_steps, "avg_ms": ms / cnt}
-        if kname in per_launch_bytes:
-            entry["algorithmic_GBps"] = per_launch_bytes[kname] / (ms / cnt * 1e-3) / 1e9
+        if kname in per_step_bytes:
+            entry["algorithmic_GBps"] = per_step_bytes[kname] / (ms / inst_steps * 1e-3) / 1e9
             entry["frac_of_hbm_peak"] = entry["algorithmic_GBps"] / hbm_peak
         if kname == "beam_sum":
             entry["algorithmic_TFLOPs"] = 8.0 * n_beams * m2 * n_probes * inst_steps / (ms * 1e-3) / 1e12
         kernels[kname] = entry
     top = max(kernels, key=lambda n: kernels[n]["ms_per_step"])
-    if top in per_launch_bytes:
+    if top in per_step_bytes:
         ach = kernels[top]["algorithmic_GBps"]
         roofline = {"kernel": top, "bound": "hbm", "achieved": ach, "peak": hbm_peak, "unit": "GB/s",
                     "frac": ach / hbm_peak, "traffic": measured_traffic(w.name, top), "peak_source": peak_src,
-                    "bytes_per_launch": per_launch_bytes[top]}
+                    "bytes_per_launch": per_step_bytes[top] / kernels[top]["launches_per_step"]}
     else:
         ach = kernels[top].get("algorithmic_TFLOPs", 0.0)
         roofline = {"kernel": top, "bound": "alu", "achieved": ach, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",

@@ -35,10 +35,10 @@ static int cuda_fail(cudaError_t e, const char* what)
 // CUDA events around every launch, on the stream the kernel is launched on.
 enum KernelClass { K_POTENTIAL = 0, K_TRANSMISSION, K_ROW_INIT, K_ROW_STEP, K_ROW_FINAL, K_COL_STEP,
                    K_BEAM_SUM, K_WIN_ROW_FFT, K_WIN_COL_ABS2, K_BIN_REDUCE, K_COL_MS_INIT, K_COL_MS_FINAL,
-                   K_LATTICE_DFT, K_PATTERNS, K_DETECTORS, K_ACCUMULATE, K_NUM_CLASSES };
+                   K_LATTICE_DFT, K_PATTERNS, K_DETECTORS, K_ACCUMULATE, K_WINDOW_OUT, K_NUM_CLASSES };
 static const char* const kClassNames[K_NUM_CLASSES] = {
     "potential", "transmission", "row_init", "row_step", "row_final", "col_step", "beam_sum",
-    "win_row_fft", "win_col_abs2", "bin_reduce", "col_ms_init", "col_ms_final", "lattice_dft", "patterns", "detectors", "accumulate" };
+    "win_row_fft", "win_col_abs2", "bin_reduce", "col_ms_init", "col_ms_final", "lattice_dft", "patterns", "detectors", "accumulate", "window_out" };
 struct TimedLaunch { int cls; cudaEvent_t e0, e1; };
 // The record is process-wide and guarded by a mutex that is taken only while timing is enabled.
 static std::atomic<bool> g_timing{false};
@@ -1039,23 +1039,19 @@ static int prism_output_impl(const prism_params* p, const void* s, const int32_t
             g.mx = mx; g.my = my; g.probe0 = p0; g.n_probes_batch = np; g.probes_x = p->probes_x;
             LAUNCH(K_BEAM_SUM, launch_beam_sum(g, st), st);
         }
-        RowArgs ra;
-        std::memset(&ra, 0, sizeof(ra));
-        ra.a = L.w; ra.out = L.w; ra.tw_x = L.tw_x; ra.tw_y = L.tw_y; ra.n_waves = np; ra.nx = mx; ra.ny = my; ra.scale = 1.f;
-        LAUNCH(K_WIN_ROW_FFT, launch_row_pass(ROW_FFT, ra, st), st);
-        ColArgs ca;
-        std::memset(&ca, 0, sizeof(ca));
-        ca.a = L.w; ca.intensity = L.intensity; ca.tw_y = L.tw_y; ca.n_waves = np; ca.nx = mx; ca.ny = my;
-        ca.scale = (float)(1.0 / (double)npix);
-        LAUNCH(K_WIN_COL_ABS2, launch_col_pass(COL_ABS2, ca, st), st);
+        // window -> FFT2 -> |.|^2 / (mx my) -> rings, on chip (window_out.cu); the patterns go to HBM only when the
+        // caller asked for them or for mask detectors
+        WindowArgs wa;
+        wa.w = L.w; wa.tw_x = L.tw_x; wa.tw_y = L.tw_y; wa.bin_start = L.bin_start; wa.bin_pix = L.bin_pix;
+        wa.out = out ? d_out + (size_t)p0 * nb : nullptr;
+        wa.intensity = (patterns || det.out) ? L.intensity : nullptr;
+        wa.n = np; wa.mx = mx; wa.my = my; wa.n_bins = nb; wa.scale = (float)(1.0 / (double)npix);
+        LAUNCH(K_WINDOW_OUT, launch_window_out(wa, st), st);
         if (patterns)
             LAUNCH(K_PATTERNS, launch_transpose_patterns(L.intensity, patterns + (size_t)p0 * npix, mx, my, np, st), st);
         if (det.out)
             LAUNCH(K_DETECTORS, launch_mask_dot(L.intensity, det.masks, det.n_masks, mx, my,
                                                 det.out + (size_t)p0 * det.n_masks, np, st), st);
-        if (out)
-            LAUNCH(K_BIN_REDUCE, launch_bin_reduce(L.intensity, (int64_t)npix, L.bin_start, L.bin_pix, nb,
-                                     d_out + (size_t)p0 * nb, np, st), st);
     }
     return out ? copy_out(p, out, L.out_stage, out_dev, st) : PRISM_OK;
 }

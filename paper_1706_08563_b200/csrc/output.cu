@@ -97,19 +97,23 @@ cudaError_t launch_beam_sum(const BeamSumArgs& g, cudaStream_t stream)
 // column FFT_Q in registers (lane = lattice row / column), (3) the results are
 // scattered to the windows, contiguous runs of pixels going to the same probe.
 // =============================================================================
+#ifndef PRISM_LATTICE_WARPS
+#define PRISM_LATTICE_WARPS 8
+#endif
 template <int Q> struct LatticeCfg {
+    static constexpr int NW = PRISM_LATTICE_WARPS, NT = NW * 32;
     static constexpr int PW = 32 / Q;                 // pixels per warp
-    static constexpr int TP = 8 * PW;                 // pixels per CTA (256 threads)
+    static constexpr int TP = NW * PW;                // pixels per CTA
     static constexpr int RS = Q + 1;                  // padded row stride (complex)
     static constexpr int PS = Q * RS + (Q == 32 ? 2 : 1);   // pixel stride: conflict-free for phases 1 and 3
     static constexpr size_t SMEM = (size_t)TP * PS * sizeof(float2);
 };
 
 template <int Q>
-__global__ void __launch_bounds__(256, 2) lattice_dft_kernel(LatticeArgs g)
+__global__ void __launch_bounds__(LatticeCfg<Q>::NT, 512 / LatticeCfg<Q>::NT) lattice_dft_kernel(LatticeArgs g)
 {
     using C = LatticeCfg<Q>;
-    constexpr int TP = C::TP, RS = C::RS, PS = C::PS, CPI = 256 / TP;   // cells per iteration
+    constexpr int TP = C::TP, RS = C::RS, PS = C::PS, CPI = C::NT / TP;   // cells per iteration
     extern __shared__ float2 sm[];                    // [TP][PS]
     const int tid = threadIdx.x;
     const int tiles_x = g.nx / TP;
@@ -204,7 +208,7 @@ static cudaError_t launch_lattice_q(const LatticeArgs& g, cudaStream_t stream)
     const long long blocks = (long long)(g.nx / C::TP) * g.n_pix_rows;
     if (blocks <= 0) return cudaSuccess;
     if (blocks > 0x7fffffffLL) return cudaErrorInvalidValue;
-    lattice_dft_kernel<Q><<<(unsigned)blocks, 256, C::SMEM, stream>>>(g);
+    lattice_dft_kernel<Q><<<(unsigned)blocks, C::NT, C::SMEM, stream>>>(g);
     return cudaGetLastError();
 }
 

@@ -37,12 +37,15 @@ __device__ __forceinline__ void named_barrier(int id, int nthreads)
 
 // ---- programmatic dependent launch (PDL) ------------------------------------------------------------------
 // The slice loop is a chain of kernels in one stream, each consuming what the previous one wrote.  Launched with
-// the programmatic-stream-serialization attribute, a kernel may start (run its prologue: tables into shared
-// memory, mbarrier init) while the previous one drains; griddep_wait() then blocks until the previous grid has
-// completed and its writes are visible.  Every kernel of the chain calls griddep_wait() before touching global
-// data and before griddep_launch(), so "the previous kernel has completed" still implies all earlier ones have.
+// the programmatic-stream-serialization attribute, the next kernel's launch is prepared while the current one
+// runs and its CTAs start as soon as the last CTA of the current one has exited; griddep_wait() then blocks until
+// the previous grid has completed and its writes are visible.  Every kernel of the chain calls griddep_wait()
+// before touching global data, so "the previous kernel has completed" still implies all earlier ones have.
+// No kernel triggers its dependents early (griddepcontrol.launch_dependents): measured on the B200, an early
+// trigger keeps the launch-bound gain (MS2 32.0 k -> 36.2 k probes/s either way) but makes the HBM-bound passes
+// slower -- 2048^2 x 1201 beams x 24 slices: 845 ms with the trigger at the top of every kernel, 745 ms without
+// (and 746 ms with plain stream order); P8 165.9 -> 164.7 ms per step.
 __device__ __forceinline__ void griddep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
-__device__ __forceinline__ void griddep_launch() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 
 template <class... KArgs, class... Args>
 inline cudaError_t launch_pdl(void (*kern)(KArgs...), unsigned grid, unsigned block, size_t smem, cudaStream_t stream,
@@ -53,7 +56,11 @@ inline cudaError_t launch_pdl(void (*kern)(KArgs...), unsigned grid, unsigned bl
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
+#ifdef PRISM_NO_PDL
+    cfg.attrs = attr; cfg.numAttrs = 0;      // experiment switch: plain stream order
+#else
     cfg.attrs = attr; cfg.numAttrs = 1;
+#endif
     return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
 }
 

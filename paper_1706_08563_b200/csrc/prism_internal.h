@@ -158,6 +158,21 @@ cudaError_t launch_bin_reduce(const float* intensity, int64_t npix, const int* b
                               const int* bin_pix, int n_bins, float* out, int n_waves,
                               cudaStream_t stream);
 
+// Fused stage-2 epilogue (window_out.cu): FFT2 of every summed window, |.|^2 * scale, ring sums -- the window is read
+// once and stays in shared memory.  `out` and / or `intensity` may be null (but not both).
+struct WindowArgs {
+    const float2* w;          // [n][my][mx] summed windows
+    const float2* tw_x;       // exp(-2 pi i m / mx)
+    const float2* tw_y;       // exp(-2 pi i m / my)
+    const int*    bin_start;  // [n_bins + 1] CSR ring lists over pixel index kx * my + ky (host fp64 decisions)
+    const int*    bin_pix;
+    float*        out;        // [n][n_bins] ring sums
+    float*        intensity;  // [n][mx][my] patterns, ky contiguous (for the 4-D output and mask detectors)
+    int           n, mx, my, n_bins;
+    float         scale;      // 1 / (mx my)
+};
+cudaError_t launch_window_out(const WindowArgs& args, cudaStream_t stream);
+
 // patterns[w][ky][kx] = intensity[w][kx][ky]: the column pass writes patterns transposed (ky contiguous), the 4-D
 // output wants them in natural order
 cudaError_t launch_transpose_patterns(const float* intensity, float* patterns, int mx, int my, int n_waves,

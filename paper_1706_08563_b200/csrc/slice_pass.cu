@@ -301,7 +301,6 @@ __global__ void transmission_kernel(const float* __restrict__ v, float2* __restr
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
     griddep_wait();                          // part of the slice loop's chain of dependent launches (pipe_ptx.cuh)
-    griddep_launch();
     if (PAIRS) {
         for (; i < npix / 2; i += stride) {
             const float2 vv = reinterpret_cast<const float2*>(v)[i];

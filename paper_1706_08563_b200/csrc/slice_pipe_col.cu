@@ -91,7 +91,6 @@ __global__ void __launch_bounds__(ColCfg<P>::THREADS, 1) col_pipe_kernel(ColArgs
     SmemTwiddles<P> tw;
     tw.bind(twtab, t);
     griddep_wait();                          // the previous kernel of the slice loop has completed (pipe_ptx.cuh)
-    griddep_launch();
 
     const int xb = g.xband;
     const int tiles_half = xb / W, tiles_per_wave = 2 * tiles_half;

@@ -89,7 +89,6 @@ __global__ void __launch_bounds__(RowCfg<P, XBE>::THREADS, 1) row_pipe_kernel(Ro
     SmemTwiddles<P> tw;
     tw.bind(twtab, t);
     griddep_wait();                          // the previous kernel of the slice loop has completed (pipe_ptx.cuh)
-    griddep_launch();
 
     const long long n_lines = (long long)g.n_waves * g.ny;
     const long long n_groups = (n_lines + C::LPT - 1) / C::LPT;

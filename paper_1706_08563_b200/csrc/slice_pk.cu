@@ -79,7 +79,6 @@ __global__ void __launch_bounds__(RowPkCfg<N, XBE>::THREADS, 1) row_pk_kernel(Ro
     if (MODE != ROW_INIT && lane == 0) { mbar_init(&bars[warp], 1); mbar_fence_init(); }
     __syncthreads();
     griddep_wait();                          // the previous kernel of the slice loop has completed (pipe_ptx.cuh)
-    griddep_launch();
 
     const long long n_lines = (long long)g.n_waves * g.ny;
     const long long n_groups = (n_lines + LPW - 1) / LPW;
@@ -303,7 +302,6 @@ __global__ void __launch_bounds__(RowB8Cfg<N, XBE>::THREADS, 1) row_b8_kernel(Ro
     }
     __syncthreads();
     griddep_wait();                          // the previous kernel of the slice loop has completed (pipe_ptx.cuh)
-    griddep_launch();
 
     const int G = gridDim.x, bid = blockIdx.x;
     const size_t wave_stride = (size_t)g.ny * N;
@@ -557,7 +555,6 @@ __global__ void __launch_bounds__(ColPkCfg<N>::THREADS, 1) col_pk_kernel(ColArgs
     }
     __syncthreads();
     griddep_wait();                          // the previous kernel of the slice loop has completed (pipe_ptx.cuh)
-    griddep_launch();
 
     const int xb = g.xband;
     const int tiles_half = xb / W, tiles_per_wave = 2 * tiles_half;
@@ -736,7 +733,6 @@ __global__ void __launch_bounds__(ColB8Cfg<N>::THREADS, 1) col_b8_kernel(ColArgs
     if (LOADS && tid == 0) { mbar_init(full, 1); mbar_fence_init(); }
     __syncthreads();
     griddep_wait();                          // the previous kernel of the slice loop has completed (pipe_ptx.cuh)
-    griddep_launch();
 
     const int xb = g.xband, nx = g.nx;
     const int tiles_per_wave = 2 * xb / W;
