@@ -50,6 +50,16 @@ enum {
     PRISM_ENOLUT       = -5   /* an atom's Z has no lookup table                                                     */
 };
 
+/* One further term of the aberration function (reading R5b of DESIGN.md; "coherent wave aberrations such
+ * as defocus or spherical aberration" are the terms (1,0) and (3,0) of this expansion):
+ *   chi(q) += (2 pi / lambda) * c * (lambda |q|)^(n+1) / (n+1) * cos(m (phi - angle)),   phi = atan2(q_y, q_x).
+ * c in Angstrom, angle in radian; 1 <= n <= 8, 0 <= m <= n + 1.  Evaluated in fp64 on the host, once per beam
+ * (PRISM) or aperture pixel (multislice). */
+typedef struct prism_aberration {
+    int32_t n, m;
+    double  c, angle;
+} prism_aberration;
+
 /* The paper's parameters (cell & pixel size PAPER.md:158,:182; slice thickness :158,:200; voltage :182;
  * probe semi-angle :200,:214; interpolation factor f :86; probe grid/step :174,:200; batch_size :126;
  * memory mode :138; annular detectors :82). */
@@ -76,6 +86,8 @@ typedef struct prism_params {
                                    prism_compute_smatrix runs `batch` beams at a time in the workspace and copies
                                    their layers out; prism_compute_output / _patterns / _detectors copy the rows
                                    a batch of probe rows needs into the workspace.  Regular probe lattices only. */
+    int32_t n_aberrations;      /* further terms of chi beside C1 and C3 (0 .. 32)                           */
+    const prism_aberration* aberrations;   /* HOST array of n_aberrations terms (may be NULL when the count is 0) */
 } prism_params;
 
 /* Per-species radial table of the projected atomic potential ("precomputed lookup table for

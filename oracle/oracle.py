@@ -27,6 +27,10 @@ __all__ = [
 ]
 
 
+class _CAberration(C.Structure):
+    _fields_ = [("n", C.c_int32), ("m", C.c_int32), ("c", C.c_double), ("angle", C.c_double)]
+
+
 class _CParams(C.Structure):
     _fields_ = [
         ("lx", C.c_double), ("ly", C.c_double), ("lz", C.c_double),
@@ -34,6 +38,7 @@ class _CParams(C.Structure):
         ("dz", C.c_double), ("voltage", C.c_double), ("alpha", C.c_double),
         ("defocus", C.c_double), ("cs", C.c_double), ("f", C.c_int32),
         ("det_step", C.c_double), ("det_max", C.c_double),
+        ("n_aberr", C.c_int32), ("aberr", C.POINTER(_CAberration)),
     ]
 
 
@@ -54,11 +59,18 @@ class Params:
     f: int = 1
     det_step: float = 1e-3
     det_max: float = 0.1
+    aberrations: tuple = ()     # further terms (n, m, c [Angstrom], angle [rad]) of the aberration function (R5b)
 
     def c(self) -> _CParams:
-        return _CParams(self.lx, self.ly, self.lz, self.nx, self.ny, self.n_slices,
-                        self.dz, self.voltage, self.alpha, self.defocus, self.cs,
-                        self.f, self.det_step, self.det_max)
+        cp = _CParams(self.lx, self.ly, self.lz, self.nx, self.ny, self.n_slices,
+                      self.dz, self.voltage, self.alpha, self.defocus, self.cs,
+                      self.f, self.det_step, self.det_max, 0, None)
+        if self.aberrations:
+            arr = (_CAberration * len(self.aberrations))(*[_CAberration(int(n), int(m), float(c), float(a))
+                                                           for n, m, c, a in self.aberrations])
+            cp.n_aberr, cp.aberr = len(self.aberrations), arr
+            cp._keep = arr                      # the array must outlive the call
+        return cp
 
 
 def build(force: bool = False) -> str:

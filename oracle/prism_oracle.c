@@ -252,11 +252,21 @@ static int in_aperture(const orc_params *p, double lambda, int kx, int ky)
     return qx * qx + qy * qy <= qmax * qmax;
 }
 
-/* aberration phase (reading R5): chi(q) = pi lambda |q|^2 C1 + (pi/2) C3 lambda^3 |q|^4 */
-static double chi(const orc_params *p, double lambda, double q2)
+/* aberration phase (reading R5): chi(q) = pi lambda |q|^2 C1 + (pi/2) C3 lambda^3 |q|^4, plus (reading R5b) the
+ * listed terms (2 pi / lambda) c (lambda |q|)^(n+1) / (n+1) cos(m (phi - angle)), phi = atan2(qy, qx) */
+static double chi(const orc_params *p, double lambda, double qx, double qy)
 {
-    return ORC_PI * lambda * q2 * p->defocus
-         + 0.5 * ORC_PI * p->cs * lambda * lambda * lambda * q2 * q2;
+    double q2 = qx * qx + qy * qy;
+    double x = ORC_PI * lambda * q2 * p->defocus
+             + 0.5 * ORC_PI * p->cs * lambda * lambda * lambda * q2 * q2;
+    if (p->n_aberr > 0 && p->aberr) {
+        double theta = lambda * sqrt(q2), phi = atan2(qy, qx);
+        for (int i = 0; i < p->n_aberr; ++i) {
+            const orc_aberration *a = &p->aberr[i];
+            x += 2.0 * ORC_PI / lambda * a->c * pow(theta, a->n + 1) / (a->n + 1) * cos(a->m * (phi - a->angle));
+        }
+    }
+    return x;
 }
 
 int orc_num_aperture(const orc_params *p)
@@ -286,7 +296,7 @@ void orc_probe(const orc_params *p, double xp, double yp, orc_c128 *psi)
             orc_c128 val = c_make(0.0, 0.0);
             if (in_aperture(p, lambda, kx, ky)) {
                 double qx = kx / p->lx, qy = ky / p->ly;
-                double phase = -chi(p, lambda, qx * qx + qy * qy)
+                double phase = -chi(p, lambda, qx, qy)
                              - 2.0 * ORC_PI * (qx * xp + qy * yp);
                 val = c_expi(phase);
             }
@@ -416,7 +426,7 @@ void orc_prism_probe(const orc_params *p, const orc_c128 *s, const int32_t *beam
     for (int b = 0; b < n_beams; ++b) {
         int kx = beams[2 * b], ky = beams[2 * b + 1];
         double qx = kx / p->lx, qy = ky / p->ly;
-        double phase = -chi(p, lambda, qx * qx + qy * qy) - 2.0 * ORC_PI * (qx * xp + qy * yp);
+        double phase = -chi(p, lambda, qx, qy) - 2.0 * ORC_PI * (qx * xp + qy * yp);
         orc_c128 coef = c_expi(phase);
         const orc_c128 *layer = s + (size_t)b * n;
         for (int j = 0; j < my_n; ++j) {

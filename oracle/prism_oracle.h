@@ -30,6 +30,12 @@ typedef struct { double re, im; } orc_c128;
 /* Parameters of one simulation, the paper's own knobs
  * (cell, pixel size, slice thickness, voltage,
  *  semi-angle, probe step; interpolation factor f). */
+/* One term of the aberration function in the (n, m) expansion (reading R5b; "coherent wave
+ * aberrations such as defocus or spherical aberration" names the two rotationally symmetric terms, C1 = (1,0)
+ * and C3 = (3,0)):  chi += (2 pi / lambda) * c * (lambda |q|)^(n+1) / (n+1) * cos(m (phi - angle)),
+ * phi = atan2(q_y, q_x); c in Angstrom, angle in radian. */
+typedef struct orc_aberration { int32_t n, m; double c, angle; } orc_aberration;
+
 typedef struct orc_params {
     double  lx, ly, lz;        /* cell (Angstrom)                              */
     int32_t nx, ny;            /* grid (powers of two)                         */
@@ -40,6 +46,8 @@ typedef struct orc_params {
     double  defocus, cs;       /* C1, C3 (Angstrom)                            */
     int32_t f;                 /* PRISM interpolation factor                   */
     double  det_step, det_max; /* annular bin width / outer angle (rad)        */
+    int32_t n_aberr;           /* further aberration terms (may be 0)          */
+    const orc_aberration *aberr;
 } orc_params;
 
 /* O1  lambda (Angstrom), sigma (rad / (V Angstrom)) */

@@ -106,6 +106,11 @@ static int check_probe(const prism_params* p)
     electron_constants(p->voltage, &lambda, nullptr);
     const double qnyq = std::min(p->nx / (2.0 * p->cell[0]), p->ny / (2.0 * p->cell[1]));
     if (p->alpha / lambda >= 2.0 / 3.0 * qnyq) return PRISM_EINVAL;      // aperture must sit inside the band-limit
+    if (p->n_aberrations < 0 || p->n_aberrations > 32 || (p->n_aberrations > 0 && !p->aberrations)) return PRISM_EINVAL;
+    for (int i = 0; i < p->n_aberrations; ++i) {
+        const prism_aberration& a = p->aberrations[i];
+        if (a.n < 1 || a.n > 8 || a.m < 0 || a.m > a.n + 1) return PRISM_EINVAL;
+    }
     return PRISM_OK;
 }
 static int check_prism(const prism_params* p)
@@ -191,9 +196,19 @@ static int band_rows(const prism_params* p)
     return std::min(p->ny / 2, (kymax + 1 + 31) / 32 * 32);
 }
 
-static double aberration(const prism_params* p, double lambda, double q2)
+// chi(q) (R5, R5b): defocus and spherical aberration, plus the caller's further (n, m) terms
+static double aberration(const prism_params* p, double lambda, double qx, double qy)
 {
-    return kPi * lambda * q2 * p->defocus + 0.5 * kPi * p->cs * lambda * lambda * lambda * q2 * q2;
+    const double q2 = qx * qx + qy * qy;
+    double chi = kPi * lambda * q2 * p->defocus + 0.5 * kPi * p->cs * lambda * lambda * lambda * q2 * q2;
+    if (p->n_aberrations > 0) {
+        const double theta = lambda * std::sqrt(q2), phi = std::atan2(qy, qx);
+        for (int i = 0; i < p->n_aberrations; ++i) {
+            const prism_aberration& a = p->aberrations[i];
+            chi += 2.0 * kPi / lambda * a.c * std::pow(theta, a.n + 1) / (a.n + 1) * std::cos(a.m * (phi - a.angle));
+        }
+    }
+    return chi;
 }
 
 // exp(-2 pi i k pos / length) for every probe coordinate and every listed index k
@@ -953,7 +968,7 @@ static int prism_output_impl(const prism_params* p, const void* s, const int32_t
     for (int b = 0; b < n_beams; ++b) {
         kxs[b] = beams[2 * b]; kys[b] = beams[2 * b + 1];
         const double qx = kxs[b] / p->cell[0], qy = kys[b] / p->cell[1];
-        const double chi = aberration(p, lambda, qx * qx + qy * qy);
+        const double chi = aberration(p, lambda, qx, qy);
         coef[b] = make_float2((float)(wscale * std::cos(-chi)), (float)(wscale * std::sin(-chi)));
     }
     up.add(L.coef_b, coef);
@@ -992,7 +1007,7 @@ static int prism_output_impl(const prism_params* p, const void* s, const int32_t
             const double qx = kxs[b] / p->cell[0], qy = kys[b] / p->cell[1];
             double turns = kxs[b] * (p->probe_origin[0] / p->cell[0]) + kys[b] * (p->probe_origin[1] / p->cell[1]);
             turns -= std::floor(turns);
-            const double ang = -aberration(p, lambda, qx * qx + qy * qy) - 2.0 * kPi * turns;
+            const double ang = -aberration(p, lambda, qx, qy) - 2.0 * kPi * turns;
             lcoef[b] = make_float2((float)(wscale * std::cos(ang)), (float)(wscale * std::sin(ang)));
         }
         up.add(L.lat_coef, lcoef);
@@ -1122,7 +1137,7 @@ static int multislice_impl(const prism_params* p, const float* v, float* out, fl
             const double qx = signed_freq(sx, nx) / p->cell[0], qy = signed_freq(sy, ny) / p->cell[1];
             const double q2 = qx * qx + qy * qy;
             if (q2 <= qmax * qmax) {
-                const double chi = aberration(p, lambda, q2);
+                const double chi = aberration(p, lambda, qx, qy);
                 ap[(size_t)sx * ny + sy] = make_float2((float)(amp * std::cos(-chi)), (float)(amp * std::sin(-chi)));
             }
         }

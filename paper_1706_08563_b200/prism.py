@@ -26,6 +26,11 @@ EXPORTS = ["prism_workspace_bytes", "prism_num_bins", "prism_num_beams", "prism_
            "prism_timing_enable", "prism_timing_classes", "prism_timing_class_name", "prism_timing_read"]
 
 
+class Aberration(C.Structure):
+    """``prism_aberration`` of include/prism.h."""
+    _fields_ = [("n", C.c_int32), ("m", C.c_int32), ("c", C.c_double), ("angle", C.c_double)]
+
+
 class Params(C.Structure):
     """``prism_params`` of include/prism.h (same field order and types)."""
     _fields_ = [
@@ -36,6 +41,7 @@ class Params(C.Structure):
         ("probe_origin", C.c_double * 2), ("probe_step", C.c_double * 2),
         ("det_step", C.c_double), ("det_max", C.c_double),
         ("batch", C.c_int32), ("potential_on_host", C.c_int32), ("smatrix_on_host", C.c_int32),
+        ("n_aberrations", C.c_int32), ("aberrations", C.POINTER(Aberration)),
     ]
 
 
@@ -123,6 +129,11 @@ def params_from_workload(w, **override) -> Params:
     p.det_step, p.det_max = w.det_step, w.det_max
     p.batch, p.potential_on_host = w.batch, w.potential_on_host
     p.smatrix_on_host = getattr(w, "smatrix_on_host", 0)
+    terms = tuple(getattr(w, "aberrations", ()))
+    if terms:
+        arr = (Aberration * len(terms))(*[Aberration(int(n), int(m), float(c), float(a)) for n, m, c, a in terms])
+        p.n_aberrations, p.aberrations = len(terms), arr
+        p._aberrations_keep = arr               # the host array must outlive the struct's use
     for k, v in override.items():
         setattr(p, k, v)
     return p

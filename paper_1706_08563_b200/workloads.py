@@ -47,6 +47,7 @@ class Workload:
     alpha: float           # probe semi-angle, rad
     defocus: float = 0.0   # C1, Angstrom
     cs: float = 0.0        # C3, Angstrom
+    aberrations: tuple = ()  # further terms (n, m, c [Angstrom], angle [rad]) of the aberration function
     f: int = 1             # PRISM interpolation factor
     probes_x: int = 1
     probes_y: int = 1

@@ -6,7 +6,7 @@ import oracle as O
 
 def oracle_params(w) -> O.Params:
     return O.Params(w.cell[0], w.cell[1], w.cell[2], w.nx, w.ny, w.n_slices, w.dz, w.voltage,
-                    w.alpha, w.defocus, w.cs, w.f, w.det_step, w.det_max)
+                    w.alpha, w.defocus, w.cs, w.f, w.det_step, w.det_max, tuple(w.aberrations))
 
 
 def oracle_potential(w, phonon=0):

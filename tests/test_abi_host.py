@@ -101,6 +101,11 @@ def test_argument_checks_without_a_gpu(prism):
                 dict(det_step=0.0), dict(n_slices=0), dict(voltage=-1.0)]:
         with pytest.raises(prism.PrismError):
             prism.num_beams(prism.params_from_workload(w, **bad))
+    # malformed aberration terms (n outside 1..8, m beyond n + 1)
+    for bad in [((0, 0, 1.0, 0.0),), ((9, 0, 1.0, 0.0),), ((2, 4, 1.0, 0.0),)]:
+        with pytest.raises(prism.PrismError):
+            prism.num_beams(prism.params_from_workload(w.with_(aberrations=bad)))
+    assert prism.num_beams(prism.params_from_workload(w.with_(aberrations=((1, 2, 10.0, 0.3),)))) == 89
     # window smaller than 16 x 16 is outside this build
     p = prism.params_from_workload(w, f=8)
     with pytest.raises(prism.PrismError):

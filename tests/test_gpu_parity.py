@@ -100,6 +100,32 @@ def test_multislice_parity(G, name):
     assert rel_l2(out[:, d:], ref[:, d:]) < 5 * TOL_OUT
 
 
+def test_general_aberration_terms_parity(G):
+    """Reading R5b: astigmatism, coma, three-fold astigmatism and C5 beside defocus, in the PRISM coefficients (per beam)
+    and in the multislice probe spectrum (per aperture pixel), against the oracle."""
+    terms = ((1, 2, 35.0, 0.4), (2, 1, 3.0e3, 1.1), (2, 3, 1.5e3, -0.6), (5, 0, 2.0e8, 0.0))
+    w = W.scaled_test_case(128, 4, 2, 4, alpha_mrad=25.0, defocus=30.0, seed_index=31,
+                           probe_offset=(0.21, 0.07)).with_(aberrations=terms)
+    p = oracle_params(w)
+    v = G.gpu_potential(w)
+    s, beams = G.gpu_smatrix(w, v)
+    v_ref = oracle_potential(w)
+    ref = O.prism_probes(p, O.smatrix(p, v_ref, beams), beams, w.probe_xy())
+    plain = O.prism_probes(oracle_params(w.with_(aberrations=())), O.smatrix(p, v_ref, beams), beams, w.probe_xy())
+    assert rel_l2(plain, ref) > 1e-2                                   # the terms matter in this case
+    out = G.gpu_prism_output(w, s, beams)
+    d = G.dark_field(w, p)
+    assert rel_l2(out, ref) < TOL_OUT and rel_l2(out[:, d:], ref[:, d:]) < 5 * TOL_OUT
+    out_m = G.gpu_multislice(w, v)
+    ref_m = O.multislice_probes(p, v_ref, w.probe_xy())
+    assert rel_l2(out_m, ref_m) < TOL_OUT and rel_l2(out_m[:, d:], ref_m[:, d:]) < 5 * TOL_OUT
+    # malformed terms are rejected
+    from paper_1706_08563_b200 import prism
+    for bad in [((0, 0, 1.0, 0.0),), ((9, 0, 1.0, 0.0),), ((2, 4, 1.0, 0.0),)]:
+        with pytest.raises(prism.PrismError):
+            prism.num_beams(prism.params_from_workload(w.with_(aberrations=bad)))
+
+
 def test_frozen_phonon_average_parity(G):
     """Row FP of SURVEY.md 8(a) (images are averaged over frozen-phonon configurations): three
     thermally displaced configurations of a 128^2 case, each a full GPU run atoms -> rings, averaged on the device
