@@ -325,13 +325,15 @@ def run_multislice(args, name, steps, warmup):
 
 
 # ------------------------------------------------------------------------------------------------ CUDA arm
-def run_prism(name, steps, warmup, world, rank, local, dist, want_cpu_baseline):
+def run_prism(name, steps, warmup, world, rank, local, dist, want_cpu_baseline, slices=0):
     """The PRISM line of one workload.  Returns the JSON-able dict (on every rank; rank 0 prints it)."""
     import torch
     from paper_1706_08563_b200 import prism, sharding, workloads
 
     dev = torch.device("cuda", local)
     w = workloads.get(name)
+    if slices > 0:                      # reduced depth, for profiler captures only (the line says so)
+        w = w.with_(n_slices=slices, name=f"{w.name}-first-{slices}-slices")
     p = prism.params_from_workload(w)
     lut_z, r_cut, lut_v = w.lut()
     n_beams, n_bins, n_probes = prism.num_beams(p), prism.num_bins(p), w.n_probes
@@ -542,6 +544,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="P16", choices=["PR1", "MS2", "P4", "P8", "P16"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--slices", type=int, default=0,
+                    help="run only this many slices of the workload (short runs under ncu; not a bench value)")
     ap.add_argument("--no-others", action="store_true",
                     help="skip the short runs of the other configurations reported under other_workloads")
     args = ap.parse_args()
@@ -568,8 +572,10 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
     line = run_prism(args.workload, args.steps, args.warmup, world, rank, local, dist,
-                     want_cpu_baseline=(world == 1 and not args.no_cpu_baseline))
-    if rank == 0 and world == 1 and args.workload == "P16" and not args.no_others:
+                     want_cpu_baseline=(world == 1 and not args.no_cpu_baseline), slices=args.slices)
+    if args.slices > 0:
+        line["reduced"] = f"first {args.slices} slices only: a profiling run, not a measurement of the workload"
+    if rank == 0 and world == 1 and args.workload == "P16" and not args.no_others and args.slices == 0:
         # the other BASELINE.json configurations, short runs on the same box (context; the line above is the headline)
         others = {}
         for other in ("P8", "P4"):

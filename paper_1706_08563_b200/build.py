@@ -14,7 +14,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libprism_b200.so")
-SOURCES = ["api.cu", "slice_pass.cu", "slice_pipe_row.cu", "slice_pipe_col.cu", "slice_pk.cu", "output.cu", "window_out.cu", "potential.cu"]
+SOURCES = ["api.cu", "slice_pass.cu", "slice_pipe_row.cu", "slice_pipe_col.cu", "slice_pk.cu", "output.cu", "window_out.cu", "ms_resident.cu", "potential.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden"]
 

@@ -35,10 +35,10 @@ static int cuda_fail(cudaError_t e, const char* what)
 // CUDA events around every launch, on the stream the kernel is launched on.
 enum KernelClass { K_POTENTIAL = 0, K_TRANSMISSION, K_ROW_INIT, K_ROW_STEP, K_ROW_FINAL, K_COL_STEP,
                    K_BEAM_SUM, K_WIN_ROW_FFT, K_WIN_COL_ABS2, K_BIN_REDUCE, K_COL_MS_INIT, K_COL_MS_FINAL,
-                   K_LATTICE_DFT, K_PATTERNS, K_DETECTORS, K_ACCUMULATE, K_WINDOW_OUT, K_NUM_CLASSES };
+                   K_LATTICE_DFT, K_PATTERNS, K_DETECTORS, K_ACCUMULATE, K_WINDOW_OUT, K_MS_RESIDENT, K_NUM_CLASSES };
 static const char* const kClassNames[K_NUM_CLASSES] = {
     "potential", "transmission", "row_init", "row_step", "row_final", "col_step", "beam_sum",
-    "win_row_fft", "win_col_abs2", "bin_reduce", "col_ms_init", "col_ms_final", "lattice_dft", "patterns", "detectors", "accumulate", "window_out" };
+    "win_row_fft", "win_col_abs2", "bin_reduce", "col_ms_init", "col_ms_final", "lattice_dft", "patterns", "detectors", "accumulate", "window_out", "ms_resident" };
 struct TimedLaunch { int cls; cudaEvent_t e0, e1; };
 // The record is process-wide and guarded by a mutex that is taken only while timing is enabled.
 static std::atomic<bool> g_timing{false};
@@ -437,27 +437,38 @@ static void carve_feeder(Arena& a, const prism_params* p, SliceFeeder& f, bool m
 
 // ---- layouts -----------------------------------------------------------------------------------------
 // beams per batch of prism_compute_smatrix: all of them when S is device memory (it is the wave buffer); with S in
-// host memory the batch lives in the workspace: p->batch beams, by default about 8 GiB of waves
+// host memory the batch lives in the workspace: p->batch beams, by default about 4 GiB of waves (two such buffers
+// alternate, so that the copy-out of one batch overlaps the propagation of the next)
 static int smatrix_batch(const prism_params* p, int n_beams)
 {
     if (p->batch > 0) return std::min<int>(p->batch, n_beams);
     if (!p->smatrix_on_host) return n_beams;
+    // at least four batches, so that the copy-out of one overlaps the propagation of the next
     const long long per_beam = (long long)p->nx * p->ny * (long long)sizeof(float2);
-    return (int)std::max<long long>(1, std::min<long long>(n_beams, (long long)(8ull << 30) / per_beam));
+    const long long by_mem = std::max<long long>(1, (long long)(4ull << 30) / per_beam);
+    return (int)std::max<long long>(1, std::min<long long>(by_mem, (n_beams + 3) / 4));
 }
 // Grids on the blocked mixed-space layout (blocked_grid): the last row pass turns blocked mixed space into natural
 // real space, which cannot be done in place, so it runs FINAL_CHUNK waves at a time into a staging buffer that is
-// then copied over the waves' own storage (or straight to a host S-matrix).
+// then copied over the waves' own storage (or straight to a host S-matrix, from two alternating staging buffers).
 constexpr int FINAL_CHUNK = 16;
-struct SmatrixLayout { SliceTables tab; SliceFeeder feed; int2* beams; float2* wave; float2* final_stage; int final_chunk; };
+struct SmatrixLayout {
+    SliceTables tab; SliceFeeder feed; int2* beams;
+    float2* wave; int wave_bufs;                 // S in host memory: wave_bufs batches of waves
+    float2* final_stage; int final_chunk, final_bufs;
+};
 static void layout_smatrix(Arena& a, const prism_params* p, int n_beams, SmatrixLayout& L)
 {
+    const bool blocked = blocked_grid(p->nx, p->ny), on_host = p->smatrix_on_host != 0;
+    const int batch = smatrix_batch(p, n_beams);
     carve_slice_tables(a, p, L.tab);
-    carve_feeder(a, p, L.feed, p->smatrix_on_host != 0 && smatrix_batch(p, n_beams) < n_beams);
+    carve_feeder(a, p, L.feed, on_host && batch < n_beams);
     L.beams = a.take<int2>(n_beams);
-    L.wave = p->smatrix_on_host ? a.take<float2>((size_t)smatrix_batch(p, n_beams) * p->nx * p->ny) : nullptr;
-    L.final_chunk = blocked_grid(p->nx, p->ny) ? std::min(FINAL_CHUNK, std::max(1, n_beams)) : 0;
-    L.final_stage = L.final_chunk ? a.take<float2>((size_t)L.final_chunk * p->nx * p->ny) : nullptr;
+    L.wave_bufs = !on_host ? 0 : (blocked || batch >= n_beams) ? 1 : 2;
+    L.wave = on_host ? a.take<float2>((size_t)L.wave_bufs * batch * p->nx * p->ny) : nullptr;
+    L.final_chunk = blocked ? std::min(FINAL_CHUNK, std::max(1, n_beams)) : 0;
+    L.final_bufs = !blocked ? 0 : on_host ? 2 : 1;
+    L.final_stage = blocked ? a.take<float2>((size_t)L.final_bufs * L.final_chunk * p->nx * p->ny) : nullptr;
 }
 
 constexpr int LATTICE_MAX_SLOTS = 4, LATTICE_MAX_Q = 32;
@@ -475,14 +486,18 @@ static void layout_output(Arena& a, const prism_params* p, int n_beams, OutputLa
     L.batch = default_probe_batch(p, npix * 12);
     L.slab = nullptr; L.slab_rows = 0;
     if (p->smatrix_on_host) {
-        // S in host memory: a batch is whole probe rows, and the workspace holds the pixel rows of every layer that
-        // those rows' windows cover (at most ~16 GiB: fewer probe rows per batch otherwise)
+        // S in host memory: a batch is whole probe rows, and the workspace holds a ring of the pixel rows of every layer
+        // that the current and the next batch's windows cover (at most ~16 GiB: fewer probe rows per batch otherwise),
+        // so the copies of batch k + 1 run while batch k computes and every row is copied once per sweep
         const int sy = std::max(1, (int)std::floor(p->probe_step[1] / (p->cell[1] / p->ny) + 0.5));
         int rows = std::min(p->probes_y, std::max(1, L.batch / std::max(1, p->probes_x)));
-        auto slab_rows = [&](int r) { return std::min(p->ny, sy * (r - 1) + my); };
-        while (rows > 1 && (size_t)n_beams * slab_rows(rows) * p->nx * sizeof(float2) > ((size_t)16 << 30)) rows /= 2;
+        auto ring_rows = [&](int r) {
+            const int pix = std::min(p->ny, sy * (r - 1) + my);                   // rows of one batch
+            return r >= p->probes_y ? pix : pix + std::min(pix, sy * r);         // + the rows the next batch adds
+        };
+        while (rows > 1 && (size_t)n_beams * ring_rows(rows) * p->nx * sizeof(float2) > ((size_t)16 << 30)) rows /= 2;
         L.batch = rows * p->probes_x;
-        L.slab_rows = slab_rows(rows);
+        L.slab_rows = ring_rows(rows);
     }
     L.tw_x = a.take<float2>(mx);
     L.tw_y = a.take<float2>(my);
@@ -547,19 +562,99 @@ static LatticePlan plan_lattice(const prism_params* p, const int32_t* beams, int
     return L;
 }
 
+// ---- S-matrix in host memory, stage 2 ("the current S-matrix subset") -----------------------------
+// The device holds a ring of pixel rows of every layer.  Rows are numbered by the unwrapped offset u from the first
+// window row of probe row 0 (pixel row (y00 + u) mod ny); probe-row batch k needs u in [sy R k, sy R k + pix_k) and
+// row u sits at ring row u % cap.  Each batch copies only the rows the ring does not hold yet, on a private copy
+// stream: with cap >= rows of a batch + rows the next batch adds, the copies of batch k + 1 overlap the kernels of
+// batch k (they wait for batch k - 1, whose rows they overwrite).
+struct SlabRing {
+    const char* s = nullptr;            // host S-matrix [n_beams][ny][nx] complex64
+    char* slab = nullptr;               // device ring [n_beams][cap][nx]
+    int cap = 0, n_beams = 0, nx = 0, ny = 0, my = 0, sy = 1, y00 = 0, rows_per_batch = 1, probes_y = 0;
+    long long have_hi = -1;             // rows [.., have_hi) of the newest batch are in the ring or on their way
+    cudaStream_t main_stream = nullptr, copy_stream = nullptr;
+    std::vector<cudaEvent_t> copied, done;
+
+    int n_batches() const { return (probes_y + rows_per_batch - 1) / rows_per_batch; }
+    int u_first(int k) const { return sy * rows_per_batch * k; }
+    int pix_rows(int k) const
+    {
+        const int r = std::min(rows_per_batch, probes_y - k * rows_per_batch);
+        return std::min(ny, sy * (r - 1) + my);
+    }
+    int init()
+    {
+        CU(cudaStreamCreateWithFlags(&copy_stream, cudaStreamNonBlocking));
+        copied.assign(n_batches(), nullptr);
+        done.assign(n_batches(), nullptr);
+        for (int k = 0; k < n_batches(); ++k) {
+            CU(cudaEventCreateWithFlags(&copied[k], cudaEventDisableTiming));
+            CU(cudaEventCreateWithFlags(&done[k], cudaEventDisableTiming));
+        }
+        // the ring may still be in use by earlier work on the main stream
+        cudaEvent_t start;
+        CU(cudaEventCreateWithFlags(&start, cudaEventDisableTiming));
+        CU(cudaEventRecord(start, main_stream));
+        CU(cudaStreamWaitEvent(copy_stream, start, 0));
+        CU(cudaEventDestroy(start));
+        return PRISM_OK;
+    }
+    // enqueue the copies batch k still needs; called in batch order, batch k + 1 right after batch k's kernel
+    int copy_batch(int k)
+    {
+        const long long a = u_first(k), b = a + pix_rows(k);
+        if (b - a > cap) return PRISM_ENOMEM;
+        long long c0 = std::max(a, have_hi < 0 ? a : have_hi);
+        // rows [c0 - cap, b - cap) are overwritten: wait for the newest earlier batch that still reads any of them
+        for (int j = k - 1; j >= 0; --j)
+            if (b - cap > u_first(j)) { CU(cudaStreamWaitEvent(copy_stream, done[j], 0)); break; }
+        const size_t row_bytes = (size_t)nx * sizeof(float2);
+        for (long long u = c0; u < b;) {
+            const int slot = (int)(u % cap), y = (int)((y00 + u) % ny);
+            const long long seg = std::min<long long>(std::min<long long>(b - u, cap - slot), ny - y);
+            CU(cudaMemcpy2DAsync(slab + (size_t)slot * row_bytes, (size_t)cap * row_bytes,
+                                 s + (size_t)y * row_bytes, (size_t)ny * row_bytes,
+                                 (size_t)seg * row_bytes, n_beams, cudaMemcpyHostToDevice, copy_stream));
+            u += seg;
+        }
+        have_hi = b;
+        CU(cudaEventRecord(copied[k], copy_stream));
+        return PRISM_OK;
+    }
+    void release()
+    {
+        for (cudaEvent_t e : copied) if (e) cudaEventDestroy(e);
+        for (cudaEvent_t e : done) if (e) cudaEventDestroy(e);
+        copied.clear(); done.clear();
+        if (copy_stream) { cudaStreamDestroy(copy_stream); copy_stream = nullptr; }
+    }
+};
+
 struct MultisliceLayout {
     SliceTables tab;
     SliceFeeder feed;
     float2 *aperture_t, *phase_x, *phase_y, *psi;
     int *bin_start, *bin_pix;
     float *intensity, *out_stage;
-    int batch;
+    int batch, waves;
 };
+// plain multislice runs resident (ms_resident.cu: one probe per SM, one launch for all slices) when the grid is one
+// of its sizes and the transmission functions of all slices are kept in device memory
+static bool multislice_resident(const prism_params* p)
+{
+    return resident_grid(p->nx, p->ny) && !p->potential_on_host &&
+           (size_t)p->n_slices * p->nx * p->ny * sizeof(float2) <= ((size_t)256 << 20);
+}
 static void layout_multislice(Arena& a, const prism_params* p, MultisliceLayout& L)
 {
     const size_t npix = (size_t)p->nx * p->ny;
     const int nb = prism_num_bins(p);
     L.batch = default_probe_batch(p, npix * 12);
+    // wave slots: a batch of the per-pass path, or one per SM for the resident kernel
+    L.waves = L.batch;
+    if (multislice_resident(p))
+        L.waves = std::max<long long>(L.batch, std::min<long long>((long long)p->probes_x * p->probes_y, RESIDENT_SLOTS));
     carve_slice_tables(a, p, L.tab);
     carve_feeder(a, p, L.feed, true);
     L.aperture_t = a.take<float2>(npix);
@@ -567,8 +662,8 @@ static void layout_multislice(Arena& a, const prism_params* p, MultisliceLayout&
     L.phase_y = a.take<float2>((size_t)p->probes_y * p->ny);
     L.bin_start = a.take<int>(nb + 1);
     L.bin_pix = a.take<int>(npix);
-    L.psi = a.take<float2>((size_t)L.batch * npix);
-    L.intensity = a.take<float>((size_t)L.batch * npix);
+    L.psi = a.take<float2>((size_t)L.waves * npix);
+    L.intensity = a.take<float>((size_t)L.waves * npix);
     L.out_stage = a.take<float>((size_t)p->probes_x * p->probes_y * nb);
 }
 
@@ -852,12 +947,48 @@ int prism_compute_smatrix(const prism_params* p, const float* v, int32_t* beams_
     const int batch = smatrix_batch(p, n_beams);
     const bool s_on_host = p->smatrix_on_host != 0;
     const bool blocked = blocked_grid(p->nx, p->ny);
+    // S in host memory: finished layers leave over a private copy stream from one of two alternating
+    // buffers (wave batches, or ROW_FINAL staging chunks on blocked grids) while the next batch / chunk is computed
+    struct CopyOut {
+        cudaStream_t stream = nullptr;
+        cudaEvent_t ready[2] = {nullptr, nullptr}, freed[2] = {nullptr, nullptr};
+        bool used[2] = {false, false};
+        ~CopyOut()
+        {
+            for (int i = 0; i < 2; ++i) { if (ready[i]) cudaEventDestroy(ready[i]); if (freed[i]) cudaEventDestroy(freed[i]); }
+            if (stream) cudaStreamDestroy(stream);
+        }
+    } out;
+    if (s_on_host) {
+        cudaError_t ce = cudaStreamCreateWithFlags(&out.stream, cudaStreamNonBlocking);
+        for (int i = 0; i < 2 && ce == cudaSuccess; ++i) {
+            ce = cudaEventCreateWithFlags(&out.ready[i], cudaEventDisableTiming);
+            if (ce == cudaSuccess) ce = cudaEventCreateWithFlags(&out.freed[i], cudaEventDisableTiming);
+        }
+        if (ce != cudaSuccess) { feed.release(); return cuda_fail(ce, "copy-out stream"); }
+    }
+    // buffer i is about to be overwritten on the main stream / has just been filled and may leave
+    auto acquire = [&](int i) -> int {
+        if (out.used[i]) CU(cudaStreamWaitEvent(st, out.freed[i], 0));
+        return PRISM_OK;
+    };
+    auto send = [&](int i, void* dst, const void* src, size_t bytes) -> int {
+        CU(cudaEventRecord(out.ready[i], st));
+        CU(cudaStreamWaitEvent(out.stream, out.ready[i], 0));
+        CU(cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, out.stream));
+        CU(cudaEventRecord(out.freed[i], out.stream));
+        out.used[i] = true;
+        return PRISM_OK;
+    };
     auto run = [&]() -> int {
-        for (int b0 = 0; b0 < n_beams; b0 += batch) {
+        int n_batch = 0, n_chunk = 0;
+        for (int b0 = 0; b0 < n_beams; b0 += batch, ++n_batch) {
             const int nb = std::min(batch, n_beams - b0);
+            const int wbuf = L.wave_bufs == 2 ? n_batch % 2 : 0;
             RowArgs ra;
-            // S in host memory (PAPER.md:136): the batch is propagated in the workspace and its layers copied out
-            ra.a = s_on_host ? L.wave : (float2*)s + (size_t)b0 * npix; ra.out = ra.a; ra.t = feed.tbuf;
+            // S in host memory: the batch is propagated in the workspace and its layers copied out
+            ra.a = s_on_host ? L.wave + (size_t)wbuf * batch * npix : (float2*)s + (size_t)b0 * npix;
+            ra.out = ra.a; ra.t = feed.tbuf;
             ra.tw_x = L.tab.tw_x; ra.tw_y = L.tab.tw_y; ra.beams = L.beams + b0;
             ra.n_waves = nb; ra.nx = p->nx; ra.ny = p->ny; ra.scale = 1.f; ra.xband = xband;
             ra.blocked = blocked ? 1 : 0;
@@ -866,10 +997,11 @@ int prism_compute_smatrix(const prism_params* p, const float* v, int32_t* beams_
             ca.xband = xband; ca.yband = yband; ca.blocked = ra.blocked;
             ca.a = ra.a; ca.tw_y = L.tab.tw_y; ca.prop_x = L.tab.prop_x; ca.prop_y = L.tab.prop_y;
             ca.ky_lim = L.tab.ky_lim; ca.n_waves = nb; ca.nx = p->nx; ca.ny = p->ny; ca.scale = 1.f;
+            int r;
+            if (s_on_host && !blocked && (r = acquire(wbuf))) return r;
             feed.begin_sweep();
             for (int sl = 0; sl < p->n_slices; ++sl) {
-                int r = feed.get(sl);
-                if (r) return r;
+                if ((r = feed.get(sl))) return r;
                 ra.t = feed.current;
                 if (sl == 0) {
                     ra.scale = (float)p->nx;                 // keeps A' = nx * FFT_x(t psi), see DESIGN.md
@@ -882,25 +1014,30 @@ int prism_compute_smatrix(const prism_params* p, const float* v, int32_t* beams_
             ra.scale = 1.0f / (float)p->nx;
             if (!blocked) {
                 LAUNCH(K_ROW_FINAL, launch_row_pass(ROW_FINAL, ra, st), st);
-                if (s_on_host)
-                    CU(cudaMemcpyAsync((float2*)s + (size_t)b0 * npix, L.wave, (size_t)nb * npix * sizeof(float2),
-                                       cudaMemcpyDeviceToHost, st));
+                if (s_on_host && (r = send(wbuf, (float2*)s + (size_t)b0 * npix, ra.a, (size_t)nb * npix * sizeof(float2))))
+                    return r;
             } else {
-                // blocked mixed space -> natural real space through the staging buffer, a few waves at a time
-                for (int c0 = 0; c0 < nb; c0 += L.final_chunk) {
+                // blocked mixed space -> natural real space through a staging buffer, a few waves at a time
+                for (int c0 = 0; c0 < nb; c0 += L.final_chunk, ++n_chunk) {
                     const int nc = std::min(L.final_chunk, nb - c0);
+                    const int sbuf = L.final_bufs == 2 ? n_chunk % 2 : 0;
+                    float2* stage = L.final_stage + (size_t)sbuf * L.final_chunk * npix;
                     RowArgs rf = ra;
-                    rf.a = ra.a + (size_t)c0 * npix; rf.out = L.final_stage; rf.n_waves = nc;
+                    rf.a = ra.a + (size_t)c0 * npix; rf.out = stage; rf.n_waves = nc;
+                    if (s_on_host && (r = acquire(sbuf))) return r;
                     LAUNCH(K_ROW_FINAL, launch_row_pass(ROW_FINAL, rf, st), st);
-                    if (s_on_host)
-                        CU(cudaMemcpyAsync((float2*)s + (size_t)(b0 + c0) * npix, L.final_stage,
-                                           (size_t)nc * npix * sizeof(float2), cudaMemcpyDeviceToHost, st));
-                    else
-                        CU(cudaMemcpyAsync(rf.a, L.final_stage, (size_t)nc * npix * sizeof(float2),
-                                           cudaMemcpyDeviceToDevice, st));
+                    if (s_on_host) {
+                        if ((r = send(sbuf, (float2*)s + (size_t)(b0 + c0) * npix, stage, (size_t)nc * npix * sizeof(float2))))
+                            return r;
+                    } else {
+                        CU(cudaMemcpyAsync(rf.a, stage, (size_t)nc * npix * sizeof(float2), cudaMemcpyDeviceToDevice, st));
+                    }
                 }
             }
         }
+        // the call's work is complete on `st` only when the last layers have left
+        for (int i = 0; i < 2; ++i)
+            if (out.used[i]) CU(cudaStreamWaitEvent(st, out.freed[i], 0));
         return PRISM_OK;
     };
     rc = run();
@@ -1018,6 +1155,14 @@ static int prism_output_impl(const prism_params* p, const void* s, const int32_t
 
     const int n_probes = p->probes_x * p->probes_y;
     const int batch = lat.ok ? rows_per_batch * p->probes_x : L.batch;
+    SlabRing ring;
+    if (s_on_host) {
+        ring.s = (const char*)s; ring.slab = (char*)L.slab; ring.cap = L.slab_rows; ring.n_beams = n_beams;
+        ring.nx = p->nx; ring.ny = p->ny; ring.my = my; ring.sy = 1 << lat.sy_log2; ring.y00 = wy0[0];
+        ring.rows_per_batch = rows_per_batch; ring.probes_y = p->probes_y; ring.main_stream = st;
+        if ((rc = ring.init())) { ring.release(); return rc; }
+    }
+    struct RingGuard { SlabRing& r; ~RingGuard() { r.release(); } } ring_guard{ring};
     for (int p0 = 0; p0 < n_probes; p0 += batch) {
         const int np = std::min(batch, n_probes - p0);
         if (lat.ok) {
@@ -1030,23 +1175,22 @@ static int prism_output_impl(const prism_params* p, const void* s, const int32_t
             const int sy = 1 << lat.sy_log2;
             g.row0 = (int)(((long long)g.py0 * sy) % p->ny);
             g.n_pix_rows = std::min(p->ny, sy * (g.n_rows - 1) + my);
-            g.slab = 0;
+            g.slab = 0; g.slab_cap = 0; g.slab_u0 = 0;
             if (s_on_host) {
-                // the job brings in the S-matrix subset it needs -- the pixel rows this batch of probe
-                // rows covers, of every layer, in one strided copy (two when the rows wrap around the cell)
-                if (g.n_pix_rows > L.slab_rows) return PRISM_ENOMEM;
-                const size_t row_bytes = (size_t)p->nx * sizeof(float2);
-                const int y_start = (wy0[0] + g.row0) % p->ny;
-                const int first = std::min(g.n_pix_rows, p->ny - y_start);
-                const size_t dpitch = (size_t)g.n_pix_rows * row_bytes, spitch = (size_t)p->ny * row_bytes;
-                CU(cudaMemcpy2DAsync(L.slab, dpitch, (const char*)s + (size_t)y_start * row_bytes, spitch,
-                                     (size_t)first * row_bytes, n_beams, cudaMemcpyHostToDevice, st));
-                if (first < g.n_pix_rows)
-                    CU(cudaMemcpy2DAsync((char*)L.slab + (size_t)first * row_bytes, dpitch, s, spitch,
-                                         (size_t)(g.n_pix_rows - first) * row_bytes, n_beams, cudaMemcpyHostToDevice, st));
-                g.s = L.slab; g.slab = 1;
+                const int k = p0 / batch;
+                int r;
+                if (k == 0 && (r = ring.copy_batch(0))) return r;
+                CU(cudaStreamWaitEvent(st, ring.copied[k], 0));
+                g.s = L.slab; g.slab = 1; g.slab_cap = ring.cap; g.slab_u0 = ring.u_first(k);
             }
             LAUNCH(K_LATTICE_DFT, launch_lattice_dft(g, st), st);
+            if (s_on_host) {
+                // the rows of the next batch come in over the copy stream while this batch's windows are transformed
+                const int k = p0 / batch;
+                CU(cudaEventRecord(ring.done[k], st));
+                int r;
+                if (p0 + batch < n_probes && (r = ring.copy_batch(k + 1))) return r;
+            }
         } else {
             BeamSumArgs g;
             g.s = (const float2*)s; g.w = L.w; g.coef_b = L.coef_b; g.phase_x = L.phase_x; g.phase_y = L.phase_y;
@@ -1166,7 +1310,24 @@ static int multislice_impl(const prism_params* p, const float* v, float* out, fl
     const int xband = band_columns(p);
     // the pipelined column pass writes the detector plane for in-band columns only: the rest stays zero (R12)
     if (pipelined_grid(nx, ny))
-        CU(cudaMemsetAsync(L.intensity, 0, (size_t)L.batch * npix * sizeof(float), st));
+        CU(cudaMemsetAsync(L.intensity, 0, (size_t)L.waves * npix * sizeof(float), st));
+    // resident path: rings only (patterns and mask detectors take the per-pass path, which keeps a batch of patterns)
+    const bool resident = multislice_resident(p) && feed.t_slices == p->n_slices && out && !patterns && !det.out;
+    auto run_resident = [&]() -> int {
+        for (int sl = 0; sl < p->n_slices; ++sl) {          // transmission functions of all slices, once
+            int r = feed.get(sl);
+            if (r) return r;
+        }
+        MsResidentArgs g;
+        g.psi = L.psi; g.intensity = L.intensity; g.t_stack = feed.tbuf; g.tw = L.tab.tw_x;
+        g.prop_x = L.tab.prop_x; g.prop_y = L.tab.prop_y; g.ky_lim = L.tab.ky_lim; g.aperture_t = L.aperture_t;
+        g.phase_x = L.phase_x; g.phase_y = L.phase_y; g.bin_start = L.bin_start; g.bin_pix = L.bin_pix; g.out = d_out;
+        g.n = nx; g.n_slices = p->n_slices; g.probe0 = 0; g.n_probes = n_probes; g.probes_x = p->probes_x;
+        g.n_bins = nb; g.xband = xband; g.yband = band_rows(p); g.slots = L.waves;
+        g.scale = (float)((double)ny / (double)nx);
+        LAUNCH(K_MS_RESIDENT, launch_ms_resident(g, st), st);
+        return PRISM_OK;
+    };
     auto run = [&]() -> int {
         for (int p0 = 0; p0 < n_probes; p0 += L.batch) {
             const int np = std::min(L.batch, n_probes - p0);
@@ -1203,7 +1364,7 @@ static int multislice_impl(const prism_params* p, const float* v, float* out, fl
         }
         return PRISM_OK;
     };
-    rc = run();
+    rc = resident ? run_resident() : run();
     feed.release();
     if (rc) return rc;
     return out ? copy_out(p, out, L.out_stage, out_dev, st) : PRISM_OK;

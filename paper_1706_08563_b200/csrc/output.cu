@@ -124,9 +124,9 @@ __global__ void __launch_bounds__(LatticeCfg<Q>::NT, 512 / LatticeCfg<Q>::NT) la
 
     // ---- (1) G[n][m] = sum over folded beams of c'_b S_b[y][x] ----
     {
-        // g.slab: g.s holds only the n_pix_rows pixel rows of this batch, row r of every layer at slab row r
-        const size_t layer = g.slab ? (size_t)g.nx * g.n_pix_rows : (size_t)g.nx * g.ny;
-        const float2* src = g.s + (size_t)(g.slab ? r : y) * g.nx + xt + px;
+        // g.slab: g.s is a ring of pixel rows (S itself is in host memory): row r of the batch at ring row (u0 + r) % cap
+        const size_t layer = g.slab ? (size_t)g.nx * g.slab_cap : (size_t)g.nx * g.ny;
+        const float2* src = g.s + (size_t)(g.slab ? (g.slab_u0 + r) % g.slab_cap : y) * g.nx + xt + px;
         float2* dst = sm + px * PS;
         if (g.n_slots == 1) {
 #pragma unroll 16

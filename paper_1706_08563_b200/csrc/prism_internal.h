@@ -116,6 +116,30 @@ cudaError_t launch_col_pipe(ColMode mode, const ColArgs& args, cudaStream_t stre
 inline bool packed_col(int nx, int ny) { return pipelined_grid(nx, ny) && ny == 2048; }
 cudaError_t launch_col_pk(ColMode mode, const ColArgs& args, cudaStream_t stream);
 
+// Resident multislice (ms_resident.cu): one launch carries probes probe0 .. probe0 + n_probes - 1 through all slices,
+// one probe per CTA at a time, from the probe spectrum to the ring sums.  Square grids of 256 or 512 points whose
+// transmission functions of all slices are in device memory.
+struct MsResidentArgs {
+    float2*       psi;        // [slots][n][n] wave storage, one slot per CTA
+    float*        intensity;  // [slots][n][n] detector plane, transposed (ky contiguous); out-of-band columns stay zero
+    const float2* t_stack;    // [n_slices][n][n] transmission functions
+    const float2* tw;         // exp(-2 pi i m / n)
+    const float2* prop_x;     // see ColArgs
+    const float2* prop_y;
+    const int*    ky_lim;
+    const float2* aperture_t; // [n][n] A_k exp(-i chi_k) * amplitude (transposed)
+    const float2* phase_x;    // [probes_x][n]
+    const float2* phase_y;    // [probes_y][n]
+    const int*    bin_start;  // ring lists over pixel index kx * n + ky
+    const int*    bin_pix;
+    float*        out;        // [all probes][n_bins]
+    int           n, n_slices, probe0, n_probes, probes_x, n_bins, xband, yband, slots;
+    float         scale;      // intensity scale of the last column pass
+};
+inline bool resident_grid(int nx, int ny) { return nx == ny && (nx == 256 || nx == 512); }
+constexpr int RESIDENT_SLOTS = 148;   // waves in flight: one per SM of a B200
+cudaError_t launch_ms_resident(const MsResidentArgs& args, cudaStream_t stream);
+
 // t = exp(i sigma V) for one slice (Eq. 1), fp64 sincos rounded once to fp32
 cudaError_t launch_transmission(const float* v, float2* t, double sigma, int64_t npix, bool pairs, cudaStream_t stream);
 
@@ -149,7 +173,9 @@ struct LatticeArgs {
     int           probes_x, probes_y;
     int           py0, n_rows;        // probe rows [py0, py0 + n_rows) of this batch
     int           row0, n_pix_rows;   // pixel rows y' = (row0 + r) mod ny, r < n_pix_rows, y' relative to y00
-    int           slab;               // 1: s is a slab [n_beams][n_pix_rows][nx] of exactly those rows (S in host memory)
+    int           slab;               // 1: s is a ring of pixel rows [n_beams][slab_cap][nx] (S in host memory): row r of
+                                      // the batch sits at ring row (slab_u0 + r) % slab_cap of every layer
+    int           slab_cap, slab_u0;
 };
 cudaError_t launch_lattice_dft(const LatticeArgs& args, cudaStream_t stream);
 
