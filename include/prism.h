@@ -23,9 +23,10 @@
  * synchronised that stream.  Host-side tables are built in fp64 inside each call and
  * uploaded from call-local host memory, so each compute call blocks the calling host
  * thread once, until its own table uploads have been consumed (they queue behind work
- * already on the stream); the kernels then run asynchronously.  When a potential is
- * streamed from host memory the library uses a private copy stream and events, created
- * and released inside the call; all of its copies are joined into `stream`.
+ * already on the stream); the kernels then run asynchronously.  When a potential or an
+ * S-matrix lives in host memory the library moves it over a private copy stream with
+ * events, created and released inside the call; all of its copies are joined into
+ * `stream`.
  *
  * Errors: every int-returning function returns PRISM_OK (0) or a negative code;
  * nothing aborts, nothing throws across the ABI.  There is no CPU fallback: on a
@@ -84,8 +85,10 @@ typedef struct prism_params {
     int32_t smatrix_on_host;    /* 0: S is device memory.  1: S is page-locked host memory ("the
                                    current S-matrix subset": streaming PRISM for S-matrices beyond device memory):
                                    prism_compute_smatrix runs `batch` beams at a time in the workspace and copies
-                                   their layers out; prism_compute_output / _patterns / _detectors copy the rows
-                                   a batch of probe rows needs into the workspace.  Regular probe lattices only. */
+                                   their layers out (copies overlapped with the next batch);
+                                   prism_compute_output / _patterns / _detectors keep a ring of pixel rows in the
+                                   workspace and bring in the rows the next batch of probe rows adds while the
+                                   current one computes.  Regular probe lattices only. */
     int32_t n_aberrations;      /* further terms of chi beside C1 and C3 (0 .. 32)                           */
     const prism_aberration* aberrations;   /* HOST array of n_aberrations terms (may be NULL when the count is 0) */
 } prism_params;
@@ -151,7 +154,10 @@ int prism_compute_output(const prism_params* p, const void* s, const int32_t* be
 /* Conventional multislice (Fig. 1c-e), the comparison path: every probe of the grid
  * is built in Fourier space (hard aperture, exp(-i chi), position phase; sum |psi0|^2 = 1), taken through
  * all slices by the same kernels, and |FFT2(psi_S)|^2 / (nx ny) is integrated into rings.
- *   v, out, workspace as above (workspace: PRISM_WS_MULTISLICE). */
+ *   v, out, workspace as above (workspace: PRISM_WS_MULTISLICE).
+ * Square 256- and 512-point grids with a device-resident potential of at most 256 MB of transmission functions run
+ * "resident": one launch, one probe per SM in flight from the probe spectrum to the ring sums;
+ * `batch` then plays no role.  Results do not depend on the route. */
 int multislice_compute_output(const prism_params* p, const float* v, float* out,
                               void* workspace, size_t workspace_bytes, void* cuda_stream);
 

@@ -52,6 +52,11 @@ __device__ __forceinline__ C2 cmul2(C2 a, float2 wr, float2 wi)
 {
     return { fma2(a.x, wr, neg2(mul2(a.y, wi))), fma2(a.x, wi, mul2(a.y, wr)) };
 }
+// conj(a) * w
+__device__ __forceinline__ C2 cmul2_conj(C2 a, float2 wr, float2 wi)
+{
+    return { fma2(a.x, wr, mul2(a.y, wi)), fma2(a.x, wi, neg2(mul2(a.y, wr))) };
+}
 
 template <int R> struct Dft;
 
@@ -273,20 +278,22 @@ __device__ __forceinline__ void fft_half(C2 (&p)[32], const float2* __restrict__
 template <int XBE> __device__ __forceinline__ constexpr bool kept(int e) { return e < XBE || e >= 64 - XBE; }
 
 // Radix-2 step of the DIF form: v (L1; slots not kept<IN>() are taken as exact zeros) -> p (pairs (a, b) whose
-// half-length transforms are the even and the odd outputs).
-template <class P, int IN>
+// half-length transforms are the even and the odd outputs).  CONJ: the step runs on conj(v) (an inverse transform is
+// the conjugate of the forward transform of the conjugate; the signs fold into the adds).
+template <class P, int IN, bool CONJ = false>
 __device__ __forceinline__ void dif_pre(const float2 (&v)[64], C2 (&p)[32], const float2* __restrict__ tab, int t)
 {
     const float2* tn = tab + P::TW2;
+    constexpr float S = CONJ ? -1.f : 1.f;
 #pragma unroll
     for (int e = 0; e < 32; ++e) {
         const float2 w = tn[t + P::T * e];                       // w_N^n, n = t + T e
         float2 a, d;
         if (kept<IN>(e) && kept<IN>(e + 32)) {
-            a = make_float2(v[e].x + v[e + 32].x, v[e].y + v[e + 32].y);
-            d = make_float2(v[e].x - v[e + 32].x, v[e].y - v[e + 32].y);
-        } else if (kept<IN>(e)) { a = v[e]; d = v[e]; }
-        else if (kept<IN>(e + 32)) { a = v[e + 32]; d = make_float2(-v[e + 32].x, -v[e + 32].y); }
+            a = make_float2(v[e].x + v[e + 32].x, S * v[e].y + S * v[e + 32].y);
+            d = make_float2(v[e].x - v[e + 32].x, S * v[e].y - S * v[e + 32].y);
+        } else if (kept<IN>(e)) { a = make_float2(v[e].x, S * v[e].y); d = a; }
+        else if (kept<IN>(e + 32)) { a = make_float2(v[e + 32].x, S * v[e + 32].y); d = make_float2(-a.x, -a.y); }
         else { a = make_float2(0.f, 0.f); d = a; }
         const float2 b = make_float2(fmaf(d.x, w.x, -d.y * w.y), fmaf(d.x, w.y, d.y * w.x));
         p[e] = { make_float2(a.x, b.x), make_float2(a.y, b.y) };

@@ -304,7 +304,7 @@ __global__ void __launch_bounds__(RowB8Cfg<N, XBE>::THREADS, 1) row_b8_kernel(Ro
     griddep_wait();                          // the previous kernel of the slice loop has completed (pipe_ptx.cuh)
 
     const int G = gridDim.x, bid = blockIdx.x;
-    const size_t wave_stride = (size_t)g.ny * N;
+    constexpr size_t wave_stride = (size_t)N * N;                 // blocked grids are square: ny == N
     const int xb = XBE < 32 ? XBE * T : g.xband;                 // in-band columns: [0, xb) and [N - xb, N)
     // this warp's lines: rows y = yb G + bid (yb < my_yblocks), wave groups wg < my_wgroups with waves
     // (wg WARPS + warp) LPW + l; `seq` = yb my_wgroups + wg numbers them in processing order
@@ -385,7 +385,7 @@ __global__ void __launch_bounds__(RowB8Cfg<N, XBE>::THREADS, 1) row_b8_kernel(Ro
                         else pos = kx < xb ? kx : (kx >= N - xb ? kx - (N - 2 * xb) : 0);
                         if (XBE < 32 && !pk::kept<XBE>(e)) { v[e] = make_float2(0.f, 0.f); continue; }
                         const float2 q = lbase[pos];
-                        v[e] = in_band(e) ? make_float2(q.y, q.x) : make_float2(0.f, 0.f);   // (im, re): inverse = swapped forward
+                        v[e] = in_band(e) ? q : make_float2(0.f, 0.f);
                     }
                     // the landing buffer is free once every lane has read its points
                     __syncwarp();
@@ -393,7 +393,7 @@ __global__ void __launch_bounds__(RowB8Cfg<N, XBE>::THREADS, 1) row_b8_kernel(Ro
                         if (LOADER == LAY_B8_CPA) issue(seq + 1);
                         else if (lane == 0) { fence_proxy_async(); issue(seq + 1); }
                     }
-                    pk::dif_pre<P, XBE>(v, p, tab, t);
+                    pk::dif_pre<P, XBE, true>(v, p, tab, t);       // inverse = conj of the forward transform of conj(v)
                 } else {
                     if (MODE == ROW_INIT) {
                         // plane wave exp(+2 pi i (kx x / nx + ky y / ny)) * amplitude at x = 2 j, 2 j + 1
@@ -408,15 +408,14 @@ __global__ void __launch_bounds__(RowB8Cfg<N, XBE>::THREADS, 1) row_b8_kernel(Ro
                             const float2 v0 = cmul_conj(b0, we), v1 = cmul_conj(b1, we);
                             p[e] = { make_float2(v0.x, v1.x), make_float2(v0.y, v1.y) };
                         }
-                    } else {
-#pragma unroll
-                        for (int e = 0; e < 32; ++e) p[e] = pk::cswap(p[e]);       // back from the swapped inverse
                     }
-                    // transmission function in pair layout: (re(2j), re(2j+1), im(2j), im(2j+1))
+                    // transmission function in pair layout: (re(2j), re(2j+1), im(2j), im(2j+1)); after the inverse p
+                    // holds the conjugate of the real-space line
 #pragma unroll
                     for (int e = 0; e < 32; ++e) {
                         const float4 q = trow[t + T * e];
-                        p[e] = pk::cmul2(p[e], make_float2(q.x, q.y), make_float2(q.z, q.w));
+                        if (MODE == ROW_INIT) p[e] = pk::cmul2(p[e], make_float2(q.x, q.y), make_float2(q.z, q.w));
+                        else p[e] = pk::cmul2_conj(p[e], make_float2(q.x, q.y), make_float2(q.z, q.w));
                     }
                 }
                 pk::fft_half<P>(p, tab, t, sm, sync);
@@ -426,19 +425,28 @@ __global__ void __launch_bounds__(RowB8Cfg<N, XBE>::THREADS, 1) row_b8_kernel(Ro
                 float4* dst = reinterpret_cast<float4*>(g.out + ((size_t)w * g.ny + y) * N);
                 if (active) {
 #pragma unroll
-                    for (int e = 0; e < 32; ++e)       // p holds the swapped inverse: (y, x) are (re, im)
-                        dst[t + T * e] = make_float4(p[e].y.x * g.scale, p[e].x.x * g.scale, p[e].y.y * g.scale, p[e].x.y * g.scale);
+                    for (int e = 0; e < 32; ++e)       // p holds the conjugate of the inverse
+                        dst[t + T * e] = make_float4(p[e].x.x * g.scale, -p[e].y.x * g.scale, p[e].x.y * g.scale, -p[e].y.y * g.scale);
                 }
             } else {
                 float2 v[64];
                 pk::dit_post<P, XBE>(p, v, tab, t);
                 if (active) {
+                    // compact column j = t + T e' (e' = e below the gap, e - gap above it) sits (j >> 3) tiles further
+                    // on: with T = 32 that is 4 e' tiles of N x 8 points, a compile-time stride per register slot
+                    static_assert(T % 8 == 0, "tile arithmetic");
+                    float2* rowt = row + (size_t)(t >> 3) * N * 8 + (t & 7);
 #pragma unroll
                     for (int e = 0; e < 64; ++e) {
                         if (!in_band(e)) continue;
-                        const int kx = t + T * e;
-                        const int j = (XBE < 32 ? e < XBE : kx < xb) ? kx : kx - (N - 2 * xb);      // compact column
-                        row[(size_t)(j >> 3) * g.ny * 8 + (j & 7)] = v[e];
+                        if (XBE < 32) {
+                            const int ep = e < XBE ? e : e - (64 - 2 * XBE);
+                            rowt[(size_t)ep * (T / 8) * N * 8] = v[e];
+                        } else {
+                            const int kx = t + T * e;
+                            const int j = kx < xb ? kx : kx - (N - 2 * xb);
+                            row[(size_t)(j >> 3) * N * 8 + (j & 7)] = v[e];
+                        }
                     }
                 }
             }
@@ -487,6 +495,7 @@ static cudaError_t launch_row_b8_x(const RowArgs& g, cudaStream_t stream)
     static PerDevice once{};
     if (cudaError_t e = opt_in_smem(kern, C::SMEM, once); e != cudaSuccess) return e;
     if (g.n_waves <= 0) return cudaSuccess;
+    if (g.ny != N) return cudaErrorInvalidValue;                                  // blocked grids are square
     if (MODE == ROW_FINAL && g.out == g.a) return cudaErrorInvalidValue;          // the layouts differ: not in place
     int grid = num_sms();
     if (grid > g.ny) grid = g.ny;

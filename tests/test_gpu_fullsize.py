@@ -252,3 +252,31 @@ def test_p4_end_to_end_full_oracle(G):
     assert ref[:, d:].sum() > 0
     assert e < TOL_OUT, e
     assert e_dark < 5 * TOL_OUT, e_dark
+
+
+def test_p8_end_to_end_full_oracle(G):
+    """BASELINE.json configs[3] end to end for one frozen-phonon configuration, atoms -> rings, against the FULL oracle:
+    its own potential, its own S-matrix of all 509 beams through all 50 slices at 1024^2 (25 450 beam-slices, a few
+    minutes on 16 cores, 8.5 GB of complex128) and its stage 2 (defocus 50 A) on 12 probes spread over the grid."""
+    w = W.p8()
+    p = oracle_params(w)
+    v = G.gpu_potential(w)
+    s, beams = G.gpu_smatrix(w, v)
+    out = G.gpu_prism_output(w, s, beams)
+    del s, v
+    torch.cuda.empty_cache()
+    v_ref = oracle_potential(w)
+    beams_ref = O.beams(p)
+    assert len(beams_ref) == 509
+    s_ref = O.smatrix(p, v_ref, beams_ref)
+    xy = w.probe_xy()
+    rows = spread(len(xy), 12)
+    ref = O.prism_probes(p, s_ref, beams_ref, xy[rows])
+    del s_ref
+    e = rel_l2(out[rows], ref)
+    d = G.dark_field(w, p)
+    e_dark = rel_l2(out[rows][:, d:], ref[:, d:])
+    print(f"P8 end to end vs full oracle: rings {e:.3e}, dark field {e_dark:.3e}")
+    assert ref[:, d:].sum() > 0
+    assert e < TOL_OUT, e
+    assert e_dark < 5 * TOL_OUT, e_dark
