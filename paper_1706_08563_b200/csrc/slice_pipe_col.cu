@@ -109,13 +109,16 @@ __global__ void __launch_bounds__(ColCfg<P>::THREADS, 1) col_pipe_kernel(ColArgs
         locate(k, w, kx0);
         const float2* src = g.a + (size_t)w * N * nx + kx0;
         float2* buf = bufs + (size_t)(k % C::NBUF) * C::BUF;
-        constexpr int CH = W / 2;                                 // 16-byte chunks per row
+        // 16-byte chunk q = tt + i TEAM of the tile: row q / CH, chunk q % CH of the row.  TEAM / CH rows per step, a
+        // multiple of R1, so both addresses advance by constants (no per-copy index arithmetic)
+        constexpr int CH = W / 2, STEP = C::TEAM / CH;
+        static_assert(C::TEAM % CH == 0 && STEP % P::R1 == 0, "copy pattern");
+        const int r0 = tt / CH, cc = tt % CH;
+        const float2* s0 = src + (size_t)r0 * nx + 2 * cc;
+        float2* d0 = buf + (r0 + r0 / P::R1) * W + 2 * cc;
 #pragma unroll
-        for (int i = 0; i < N * CH / C::TEAM; ++i) {
-            const int q = tt + i * C::TEAM;
-            const int row = q / CH, cc = q % CH;
-            cp_async16(buf + (row + row / P::R1) * W + 2 * cc, src + (size_t)row * nx + 2 * cc);
-        }
+        for (int i = 0; i < N / STEP; ++i)
+            cp_async16(d0 + i * (STEP + STEP / P::R1) * W, s0 + (size_t)i * STEP * nx);
         cp_async_arrive(&full[k % C::NBUF]);
     };
     if (LOADS) {
