@@ -533,7 +533,7 @@ def run_prism(name, steps, warmup, world, rank, local, dist, want_cpu_baseline, 
         "roofline": roofline, "kernels": kernels,
     }
     if want_cpu_baseline and rank == 0:
-        val, desc, cores, detail = oracle_sample(w)
+        val, desc, cores, detail = oracle_sample(w, budget_s=40.0)     # whole beams through up to 50 slices
         line["cpu_baseline"] = {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc,
                                 "extrapolated": detail["extrapolated"],
                                 "beam_slices_per_s": detail["beam_slices_per_s"]}

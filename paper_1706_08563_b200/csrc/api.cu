@@ -34,11 +34,11 @@ static int cuda_fail(cudaError_t e, const char* what)
 // Optional per-kernel-class device timing (prism_timing_enable / prism_timing_read): a pair of
 // CUDA events around every launch, on the stream the kernel is launched on.
 enum KernelClass { K_POTENTIAL = 0, K_TRANSMISSION, K_ROW_INIT, K_ROW_STEP, K_ROW_FINAL, K_COL_STEP,
-                   K_BEAM_SUM, K_WIN_ROW_FFT, K_WIN_COL_ABS2, K_BIN_REDUCE, K_COL_MS_INIT, K_COL_MS_FINAL,
+                   K_BEAM_SUM, K_BIN_REDUCE, K_COL_MS_INIT, K_COL_MS_FINAL,
                    K_LATTICE_DFT, K_PATTERNS, K_DETECTORS, K_ACCUMULATE, K_WINDOW_OUT, K_MS_RESIDENT, K_NUM_CLASSES };
 static const char* const kClassNames[K_NUM_CLASSES] = {
     "potential", "transmission", "row_init", "row_step", "row_final", "col_step", "beam_sum",
-    "win_row_fft", "win_col_abs2", "bin_reduce", "col_ms_init", "col_ms_final", "lattice_dft", "patterns", "detectors", "accumulate", "window_out", "ms_resident" };
+    "bin_reduce", "col_ms_init", "col_ms_final", "lattice_dft", "patterns", "detectors", "accumulate", "window_out", "ms_resident" };
 struct TimedLaunch { int cls; cudaEvent_t e0, e1; };
 // The record is process-wide and guarded by a mutex that is taken only while timing is enabled.
 static std::atomic<bool> g_timing{false};

@@ -56,11 +56,7 @@ inline cudaError_t launch_pdl(void (*kern)(KArgs...), unsigned grid, unsigned bl
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
-#ifdef PRISM_NO_PDL
-    cfg.attrs = attr; cfg.numAttrs = 0;      // experiment switch: plain stream order
-#else
     cfg.attrs = attr; cfg.numAttrs = 1;
-#endif
     return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
 }
 

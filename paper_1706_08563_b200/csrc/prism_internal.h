@@ -55,7 +55,6 @@ enum RowMode {
     ROW_INIT  = 0,   // plane wave b  -> * t            -> FFT_x -> A          (first slice, no read)
     ROW_STEP  = 1,   // A -> IFFT_x   -> * t            -> FFT_x -> A
     ROW_FINAL = 2,   // A -> IFFT_x   -> * scale        -> out   (real-space exit wave, S-matrix layer)
-    ROW_FFT   = 3,   // a -> FFT_x -> a                           (probe windows, stage 2)
 };
 struct RowArgs {
     float2*       a;          // [n_waves][ny][nx] in/out
@@ -90,11 +89,10 @@ enum ColMode {
     COL_STEP     = 0,   // A -> FFT_y -> * P -> IFFT_y -> A
     COL_MS_INIT  = 1,   // probe spectrum Psi0(kx, ky) -> IFFT_y -> A          (multislice start, no read)
     COL_MS_FINAL = 2,   // A -> FFT_y -> * P -> |.|^2 -> intensity[w][kx][ky]  (multislice end, no IFFT)
-    COL_ABS2     = 3,   // a -> FFT_y -> |.|^2 * scale -> intensity[w][kx][ky] (probe windows, stage 2)
 };
 struct ColArgs {
     float2*       a;          // [n_waves][ny][nx] in/out
-    float*        intensity;  // [n_waves][nx][ny]  (COL_MS_FINAL, COL_ABS2) -- transposed: ky contiguous
+    float*        intensity;  // [n_waves][nx][ny]  (COL_MS_FINAL) -- transposed: ky contiguous
     const float2* tw_y;       // exp(-2 pi i m / ny)
     const float2* prop_x;     // [nx] x-factor of the propagator (all scale factors folded in)
     const float2* prop_y;     // [ny] y-factor
@@ -108,7 +106,7 @@ struct ColArgs {
     int           xband;      // see RowArgs
     int           yband;      // a multiple of 32 with ky_lim[kx] < yband for every kx (pipelined kernels)
     int           blocked;    // 1: mixed space in the blocked layout "B8" (see RowArgs)
-    float         scale;      // COL_ABS2 / COL_MS_FINAL intensity scale
+    float         scale;      // COL_MS_FINAL intensity scale
 };
 cudaError_t launch_col_pass(ColMode mode, const ColArgs& args, cudaStream_t stream);
 cudaError_t launch_col_pipe(ColMode mode, const ColArgs& args, cudaStream_t stream);

@@ -8,8 +8,8 @@
 //   column pass (fixed kx):  FFT_y  -> * P(kx, ky)      -> IFFT_y
 // with the wave kept between passes in mixed space A[w][y][kx].  The same two
 // kernels also start and finish the plane waves of the S-matrix
-// and the probes of plain multislice, and transform the PRISM
-// probe windows.
+// and the probes of plain multislice.  (The PRISM probe windows of
+// PAPER.md:128 are transformed by window_out.cu.)
 #include "fft_core.cuh"
 #include "prism_internal.h"
 #include "pipe_ptx.cuh"
@@ -124,15 +124,14 @@ static cudaError_t launch_row_n(RowMode mode, const RowArgs& g, cudaStream_t str
         case ROW_INIT:  return launch_row_t<P, LPC, ROW_INIT>(g, stream);
         case ROW_STEP:  return launch_row_t<P, LPC, ROW_STEP>(g, stream);
         case ROW_FINAL: return launch_row_t<P, LPC, ROW_FINAL>(g, stream);
-        case ROW_FFT:   return launch_row_t<P, LPC, ROW_FFT>(g, stream);
     }
     return cudaErrorInvalidValue;
 }
 
 cudaError_t launch_row_pass(RowMode mode, const RowArgs& g, cudaStream_t stream)
 {
-    if (packed_row(g.nx, g.ny) && mode != ROW_FFT) return launch_row_pk(mode, g, stream);
-    if (pipelined_grid(g.nx, g.ny) && mode != ROW_FFT) return launch_row_pipe(mode, g, stream);
+    if (packed_row(g.nx, g.ny)) return launch_row_pk(mode, g, stream);
+    if (pipelined_grid(g.nx, g.ny)) return launch_row_pipe(mode, g, stream);
     switch (g.nx) {
         case 16:   return launch_row_n<16>(mode, g, stream);
         case 32:   return launch_row_n<32>(mode, g, stream);
@@ -267,15 +266,14 @@ static cudaError_t launch_col_n(ColMode mode, const ColArgs& g, cudaStream_t str
         case COL_STEP:     return launch_col_t<P, W, G, COL_STEP>(g, stream);
         case COL_MS_INIT:  return launch_col_t<P, W, G, COL_MS_INIT>(g, stream);
         case COL_MS_FINAL: return launch_col_t<P, W, G, COL_MS_FINAL>(g, stream);
-        case COL_ABS2:     return launch_col_t<P, W, G, COL_ABS2>(g, stream);
     }
     return cudaErrorInvalidValue;
 }
 
 cudaError_t launch_col_pass(ColMode mode, const ColArgs& g, cudaStream_t stream)
 {
-    if (packed_col(g.nx, g.ny) && mode != COL_ABS2) return launch_col_pk(mode, g, stream);
-    if (pipelined_grid(g.nx, g.ny) && mode != COL_ABS2) return launch_col_pipe(mode, g, stream);
+    if (packed_col(g.nx, g.ny)) return launch_col_pk(mode, g, stream);
+    if (pipelined_grid(g.nx, g.ny)) return launch_col_pipe(mode, g, stream);
     if (g.nx % 8 != 0) return cudaErrorInvalidValue;
     switch (g.ny) {
         case 16:   return launch_col_n<16>(mode, g, stream);

@@ -362,6 +362,36 @@ def test_single_slice_and_rectangular_probe_grid(G):
     assert rel_l2(G.gpu_multislice(w, v), O.multislice_probes(p, v_ref, w.probe_xy())) < TOL_OUT
 
 
+def test_resident_multislice_edge_cases(G):
+    """The resident multislice kernel (256^2 / 512^2 grids, one probe per SM): a single slice, more
+    probes than SMs with a ragged last round, a rectangular probe grid off the pixel lattice, empty space, and
+    agreement with the per-pass path (taken when the potential is streamed from host memory)."""
+    from paper_1706_08563_b200 import prism
+    w = W.scaled_test_case(256, 1, 2, 4, voltage=300e3, alpha_mrad=20.0, seed_index=41, density=0.1).with_(
+        probes_x=3, probes_y=5, probe_step=(1.3, 0.7), probe_origin=(0.123, 0.456))
+    p = oracle_params(w)
+    v = G.gpu_potential(w)
+    assert rel_l2(G.gpu_multislice(w, v), O.multislice_probes(p, oracle_potential(w), w.probe_xy())) < TOL_OUT
+    # 13 x 13 = 169 probes > 148 SMs, three slices; the oracle on a sample of the probes, the per-pass path on all
+    w2 = W.scaled_test_case(256, 3, 2, 13, voltage=300e3, alpha_mrad=20.0, seed_index=42, defocus=35.0)
+    p2 = oracle_params(w2)
+    v2 = G.gpu_potential(w2)
+    out = G.gpu_multislice(w2, v2)
+    pick = np.array([0, 1, 77, 147, 148, 149, 168])
+    ref = O.multislice_probes(p2, oracle_potential(w2), w2.probe_xy()[pick])
+    d = G.dark_field(w2, p2)
+    assert rel_l2(out[pick], ref) < TOL_OUT and rel_l2(out[pick][:, d:], ref[:, d:]) < 5 * TOL_OUT
+    v2_host = G.gpu_potential(w2, on_host=True)
+    per_pass = G.gpu_multislice(w2, v2_host)                        # streamed potential: launch-per-pass kernels
+    assert rel_l2(out, per_pass) < 2e-6
+    # empty space: rings = aperture pixel counts (closed form through the oracle)
+    w0 = w2.with_(atoms=np.zeros((0, 3)), z=np.zeros(0, np.int32))
+    v0 = torch.zeros((w0.n_slices, w0.ny, w0.nx), dtype=torch.float32, device=G.DEV)
+    ms0 = G.gpu_multislice(w0, v0)
+    ref0 = O.multislice_probes(oracle_params(w0), np.zeros((w0.n_slices, w0.ny, w0.nx)), w0.probe_xy()[:1])
+    assert np.max(np.abs(ms0 - ref0)) < 2e-6 and abs(ms0.sum(axis=1) - 1.0).max() < 1e-5
+
+
 def test_error_codes(G):
     from paper_1706_08563_b200 import prism
     w = CASES["PR1"]
