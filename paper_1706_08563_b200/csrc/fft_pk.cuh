@@ -129,10 +129,75 @@ template <> struct Dft<16> {
     }
 };
 
+// Twiddle w32^m = (-i)^q * cos(t) * (1 - i tan(t)) with q the nearest quarter turn and |t| <= pi/4, t = 2 pi j / 32.
+__device__ __forceinline__ constexpr int tw_q(int m) { return (m % 8 == 4) ? m / 8 : (m + 4) / 8; }
+__device__ __forceinline__ constexpr int tw_j(int m) { return m - 8 * tw_q(m); }
+// a * (-i)^q
+__device__ __forceinline__ C2 rotq(C2 a, int q)
+{
+    switch (q & 3) {
+        case 1: return { a.y, neg2(a.x) };
+        case 2: return { neg2(a.x), neg2(a.y) };
+        case 3: return { neg2(a.y), a.x };
+        default: return a;
+    }
+}
+
+#ifndef PRISM_PK_TAN_TWIDDLES
+#define PRISM_PK_TAN_TWIDDLES 1
+#endif
+
 template <> struct Dft<32> {
     __device__ __forceinline__ static void run(C2* a)
     {
         // n = 4 n1 + n2 (n1 < 8, n2 < 4); k = k1 + 8 k2.  Y[n2][k1] = DFT8 over n1, twiddle w32^(n2 k1), DFT4 over n2.
+        C2 y[4][8];
+#pragma unroll
+        for (int n2 = 0; n2 < 4; ++n2) {
+#pragma unroll
+            for (int n1 = 0; n1 < 8; ++n1) y[n2][n1] = a[4 * n1 + n2];
+            Dft<8>::run(y[n2]);
+        }
+#if PRISM_PK_TAN_TWIDDLES
+        // Scaled twiddles: y w = (-i)^q c (y (1 - i tan)) costs two FFMA2 for u = (-i)^q y (1 - i tan) -- the quarter
+        // turn is a renaming -- and the cosines ride on the adds of the radix-4 butterfly, which become FFMA2 at the
+        // same cost:  z1 + z3 = c1 (u1 + (c3 / c1) u3),  z0 + z2 = z0 + c2 u2,  out = t0 + c1 S ...
+        // 22 packed instructions per column k1 instead of 28 (three complex multiplies + 16 adds).
+        constexpr float CJ[9] = { 0.70710678118654752440f, 0.83146961230254523708f, 0.92387953251128675613f,
+                                  0.98078528040323044913f, 1.f, 0.98078528040323044913f, 0.92387953251128675613f,
+                                  0.83146961230254523708f, 0.70710678118654752440f };                 // cos(2 pi j / 32), j = -4 .. 4
+        constexpr float TJ[9] = { -1.f, -0.66817863791929891999f, -0.41421356237309504880f, -0.19891236737965800691f, 0.f,
+                                  0.19891236737965800691f, 0.41421356237309504880f, 0.66817863791929891999f, 1.f };   // tan
+        {
+            C2 z[4] = { y[0][0], y[1][0], y[2][0], y[3][0] };
+            Dft<4>::run(z);
+            a[0] = z[0]; a[8] = z[1]; a[16] = z[2]; a[24] = z[3];
+        }
+#pragma unroll
+        for (int k1 = 1; k1 < 8; ++k1) {
+            C2 u[4];
+            float c[4] = { 1.f, 1.f, 1.f, 1.f };
+#pragma unroll
+            for (int n2 = 1; n2 < 4; ++n2) {
+                const int m = n2 * k1, j = tw_j(m);
+                const float tau = TJ[j + 4];
+                c[n2] = CJ[j + 4];
+                const C2 v = y[n2][k1];
+                const C2 w = (j == 0) ? v : C2{ fma2(v.y, bc(tau), v.x), fma2(v.x, bc(-tau), v.y) };   // v (1 - i tan)
+                u[n2] = rotq(w, tw_q(m));
+            }
+            const C2 z0 = y[0][k1];
+            const C2 t0 = { fma2(u[2].x, bc(c[2]), z0.x), fma2(u[2].y, bc(c[2]), z0.y) };
+            const C2 t1 = { fma2(u[2].x, bc(-c[2]), z0.x), fma2(u[2].y, bc(-c[2]), z0.y) };
+            const float r = c[3] / c[1];
+            const C2 sp = { fma2(u[3].x, bc(r), u[1].x), fma2(u[3].y, bc(r), u[1].y) };      // (z1 + z3) / c1
+            const C2 dm = { fma2(u[3].x, bc(-r), u[1].x), fma2(u[3].y, bc(-r), u[1].y) };    // (z1 - z3) / c1
+            a[k1]      = { fma2(sp.x, bc(c[1]), t0.x), fma2(sp.y, bc(c[1]), t0.y) };
+            a[k1 + 16] = { fma2(sp.x, bc(-c[1]), t0.x), fma2(sp.y, bc(-c[1]), t0.y) };
+            a[k1 + 8]  = { fma2(dm.y, bc(c[1]), t1.x), fma2(dm.x, bc(-c[1]), t1.y) };       // t1 + (-i) c1 dm
+            a[k1 + 24] = { fma2(dm.y, bc(-c[1]), t1.x), fma2(dm.x, bc(c[1]), t1.y) };
+        }
+#else
         // w32^m = exp(-2 pi i m / 32) = (WC[m], -WS[m]) for m <= 21
         constexpr float WC[22] = { 1.f, 0.98078528040323044913f, 0.92387953251128675613f, 0.83146961230254523708f,
                                    0.70710678118654752440f, 0.55557023301960222474f, 0.38268343236508977173f,
@@ -148,13 +213,6 @@ template <> struct Dft<32> {
                                    0.38268343236508977173f, 0.19509032201612826785f, 0.f, -0.19509032201612826785f,
                                    -0.38268343236508977173f, -0.55557023301960222474f, -0.70710678118654752440f,
                                    -0.83146961230254523708f };
-        C2 y[4][8];
-#pragma unroll
-        for (int n2 = 0; n2 < 4; ++n2) {
-#pragma unroll
-            for (int n1 = 0; n1 < 8; ++n1) y[n2][n1] = a[4 * n1 + n2];
-            Dft<8>::run(y[n2]);
-        }
 #pragma unroll
         for (int n2 = 1; n2 < 4; ++n2)
 #pragma unroll
@@ -168,6 +226,7 @@ template <> struct Dft<32> {
             Dft<4>::run(z);
             a[k1] = z[0]; a[k1 + 8] = z[1]; a[k1 + 16] = z[2]; a[k1 + 24] = z[3];
         }
+#endif
     }
 };
 
