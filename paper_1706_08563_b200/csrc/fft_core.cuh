@@ -74,18 +74,93 @@ template <> struct Dft<8> {
     }
 };
 
+// ---- radix-4 butterfly over twiddled inputs, scaled-twiddle form --------------------------------------------
+// out = DFT4(z0, y1 w^k1, y2 w^(2 k1), y3 w^(3 k1)), w = exp(-2 pi i / R).  Each twiddle is written
+// w^m = (-i)^q cos(t) (1 - i tan(t)), q the nearest quarter turn, |t| <= pi/4: u = (-i)^q y (1 - i tan) costs two
+// FMAs (the quarter turn is a renaming with signs), and the cosines ride on the adds of the butterfly, which become
+// FMAs at the same cost: z1 + z3 = c1 (u1 + (c3 / c1) u3), z0 + z2 = z0 + c2 u2, out0 = t0 + c1 S, ...
+// 22 FMA-pipe operations instead of 28 (three complex multiplies and sixteen adds).  Measured: column passes 1.41 ->
+// 1.35 ms (1024 points), 0.377 -> 0.368 ms (512); resident multislice 16.8 -> 16.65 ms.  Translation units that run
+// their adds as packed FADD2 (PRISM_PACKED_ADDS: the row passes, window_out) keep the plain form: there a packed
+// version of this butterfly (11 FFMA2) cut the instruction count by 10 % and was not faster (1.50 ms at 1024 points,
+// 0.44 against 0.38 ms at 512).
+#ifndef PRISM_TAN_TWIDDLES
+#ifdef PRISM_PACKED_ADDS
+#define PRISM_TAN_TWIDDLES 0
+#else
+#define PRISM_TAN_TWIDDLES 1
+#endif
+#endif
+template <int R> __device__ __forceinline__ constexpr int tw_quarter(int m)
+{ return (m % (R / 4) == R / 8) ? m / (R / 4) : (m + R / 8) / (R / 4); }
+__device__ __forceinline__ float2 rot_quarter(float2 a, int q)      // a * (-i)^q
+{
+    switch (q & 3) {
+        case 1: return make_float2(a.y, -a.x);
+        case 2: return make_float2(-a.x, -a.y);
+        case 3: return make_float2(-a.y, a.x);
+        default: return a;
+    }
+}
+template <int R>
+__device__ __forceinline__ void twiddled_dft4(float2 z0, float2 y1, float2 y2, float2 y3, int k1,
+                                              float2& o0, float2& o1, float2& o2, float2& o3)
+{
+    static_assert(R == 16 || R == 32, "tables");
+    // cos and tan of 2 pi j / R for j = -R/8 .. R/8
+    constexpr float C16[5] = { 0.70710678118654752440f, 0.92387953251128675613f, 1.f, 0.92387953251128675613f,
+                               0.70710678118654752440f };
+    constexpr float T16[5] = { -1.f, -0.41421356237309504880f, 0.f, 0.41421356237309504880f, 1.f };
+    constexpr float C32[9] = { 0.70710678118654752440f, 0.83146961230254523708f, 0.92387953251128675613f,
+                               0.98078528040323044913f, 1.f, 0.98078528040323044913f, 0.92387953251128675613f,
+                               0.83146961230254523708f, 0.70710678118654752440f };
+    constexpr float T32[9] = { -1.f, -0.66817863791929891999f, -0.41421356237309504880f, -0.19891236737965800691f, 0.f,
+                               0.19891236737965800691f, 0.41421356237309504880f, 0.66817863791929891999f, 1.f };
+    const float2 y[4] = { z0, y1, y2, y3 };
+    float2 u[4];
+    float c[4] = { 1.f, 1.f, 1.f, 1.f };
+#pragma unroll
+    for (int n2 = 1; n2 < 4; ++n2) {
+        const int m = n2 * k1, q = tw_quarter<R>(m), j = m - q * (R / 4);
+        const float tau = R == 16 ? T16[j + 2] : T32[j + 4];
+        c[n2] = R == 16 ? C16[j + 2] : C32[j + 4];
+        const float2 v = y[n2];
+        const float2 w = (j == 0) ? v : make_float2(fmaf(v.y, tau, v.x), fmaf(v.x, -tau, v.y));     // v (1 - i tan)
+        u[n2] = rot_quarter(w, q);
+    }
+    const float2 t0 = make_float2(fmaf(u[2].x, c[2], z0.x), fmaf(u[2].y, c[2], z0.y));
+    const float2 t1 = make_float2(fmaf(u[2].x, -c[2], z0.x), fmaf(u[2].y, -c[2], z0.y));
+    const float r = c[3] / c[1];
+    const float2 sp = make_float2(fmaf(u[3].x, r, u[1].x), fmaf(u[3].y, r, u[1].y));            // (z1 + z3) / c1
+    const float2 dm = make_float2(fmaf(u[3].x, -r, u[1].x), fmaf(u[3].y, -r, u[1].y));          // (z1 - z3) / c1
+    o0 = make_float2(fmaf(sp.x, c[1], t0.x), fmaf(sp.y, c[1], t0.y));
+    o2 = make_float2(fmaf(sp.x, -c[1], t0.x), fmaf(sp.y, -c[1], t0.y));
+    o1 = make_float2(fmaf(dm.y, c[1], t1.x), fmaf(dm.x, -c[1], t1.y));                          // t1 + (-i) c1 dm
+    o3 = make_float2(fmaf(dm.y, -c[1], t1.x), fmaf(dm.x, c[1], t1.y));
+}
+
 template <> struct Dft<16> {
     __device__ __forceinline__ static void run(float2* a)
     {
         // n = 4 n1 + n2 ; k = k1 + 4 k2.  Y[n2][k1] = DFT4 over n1, then twiddle w16^(n2 k1), DFT4 over n2.
-        const float c1 = 0.92387953251128675613f, s1 = 0.38268343236508977173f;   // cos, sin(pi/8)
-        const float h  = 0.70710678118654752440f;
         float2 y[4][4];
 #pragma unroll
         for (int n2 = 0; n2 < 4; ++n2) {
             y[n2][0] = a[n2]; y[n2][1] = a[n2 + 4]; y[n2][2] = a[n2 + 8]; y[n2][3] = a[n2 + 12];
             Dft<4>::run(y[n2]);
         }
+#if PRISM_TAN_TWIDDLES
+        {
+            float2 z[4] = { y[0][0], y[1][0], y[2][0], y[3][0] };
+            Dft<4>::run(z);
+            a[0] = z[0]; a[4] = z[1]; a[8] = z[2]; a[12] = z[3];
+        }
+#pragma unroll
+        for (int k1 = 1; k1 < 4; ++k1)
+            twiddled_dft4<16>(y[0][k1], y[1][k1], y[2][k1], y[3][k1], k1, a[k1], a[k1 + 4], a[k1 + 8], a[k1 + 12]);
+#else
+        const float c1 = 0.92387953251128675613f, s1 = 0.38268343236508977173f;   // cos, sin(pi/8)
+        const float h  = 0.70710678118654752440f;
         // w16^m = exp(-2 pi i m / 16): m=1 (c1,-s1) m=2 (h,-h) m=3 (s1,-c1) m=4 (0,-1) m=6 (-h,-h) m=9 (-c1, s1)
         y[1][1] = cmul(y[1][1], make_float2(c1, -s1));
         y[1][2] = cmul(y[1][2], make_float2(h, -h));
@@ -102,6 +177,7 @@ template <> struct Dft<16> {
             Dft<4>::run(z);
             a[k1] = z[0]; a[k1 + 4] = z[1]; a[k1 + 8] = z[2]; a[k1 + 12] = z[3];
         }
+#endif
     }
 };
 
@@ -109,6 +185,23 @@ template <> struct Dft<32> {
     __device__ __forceinline__ static void run(float2* a)
     {
         // n = 4 n1 + n2 (n1 < 8, n2 < 4); k = k1 + 8 k2.  Y[n2][k1] = DFT8 over n1, twiddle w32^(n2 k1), DFT4 over n2.
+        float2 y[4][8];
+#pragma unroll
+        for (int n2 = 0; n2 < 4; ++n2) {
+#pragma unroll
+            for (int n1 = 0; n1 < 8; ++n1) y[n2][n1] = a[4 * n1 + n2];
+            Dft<8>::run(y[n2]);
+        }
+#if PRISM_TAN_TWIDDLES
+        {
+            float2 z[4] = { y[0][0], y[1][0], y[2][0], y[3][0] };
+            Dft<4>::run(z);
+            a[0] = z[0]; a[8] = z[1]; a[16] = z[2]; a[24] = z[3];
+        }
+#pragma unroll
+        for (int k1 = 1; k1 < 8; ++k1)
+            twiddled_dft4<32>(y[0][k1], y[1][k1], y[2][k1], y[3][k1], k1, a[k1], a[k1 + 8], a[k1 + 16], a[k1 + 24]);
+#else
         // w32^m = exp(-2 pi i m / 32) = (WC[m], -WS[m]) for m <= 21
         constexpr float WC[22] = { 1.f, 0.98078528040323044913f, 0.92387953251128675613f, 0.83146961230254523708f,
                                    0.70710678118654752440f, 0.55557023301960222474f, 0.38268343236508977173f,
@@ -124,13 +217,6 @@ template <> struct Dft<32> {
                                    0.38268343236508977173f, 0.19509032201612826785f, 0.f, -0.19509032201612826785f,
                                    -0.38268343236508977173f, -0.55557023301960222474f, -0.70710678118654752440f,
                                    -0.83146961230254523708f };
-        float2 y[4][8];
-#pragma unroll
-        for (int n2 = 0; n2 < 4; ++n2) {
-#pragma unroll
-            for (int n1 = 0; n1 < 8; ++n1) y[n2][n1] = a[4 * n1 + n2];
-            Dft<8>::run(y[n2]);
-        }
 #pragma unroll
         for (int n2 = 1; n2 < 4; ++n2)
 #pragma unroll
@@ -142,6 +228,7 @@ template <> struct Dft<32> {
             Dft<4>::run(z);
             a[k1] = z[0]; a[k1 + 8] = z[1]; a[k1 + 16] = z[2]; a[k1 + 24] = z[3];
         }
+#endif
     }
 };
 
