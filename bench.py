@@ -490,6 +490,20 @@ def run_prism(name, steps, warmup, world, rank, local, dist, want_cpu_baseline, 
             entry["frac_of_hbm_peak"] = entry["algorithmic_GBps"] / hbm_peak
         if kname == "beam_sum":
             entry["algorithmic_TFLOPs"] = 8.0 * n_beams * m2 * n_probes * inst_steps / (ms * 1e-3) / 1e12
+        # stage 2: the lattice kernel reads the pixel rows of a probe-row batch once and writes
+        # the summed windows; window_out reads every window once
+        if kname == "lattice_dft":
+            sy = max(1, int(round(w.probe_step[1] / (w.cell[1] / w.ny))))
+            rows_per_launch = max(1, int(round(w.probes_y * inst_steps / cnt)))
+            pix_rows = min(w.ny, sy * (rows_per_launch - 1) + w.ny // w.f)
+            lat_bytes = (cnt / inst_steps) * 8.0 * n_beams * pix_rows * w.nx + 8.0 * m2 * n_probes
+            entry["algorithmic_GBps"] = lat_bytes / (ms / inst_steps * 1e-3) / 1e9
+            entry["frac_of_hbm_peak"] = entry["algorithmic_GBps"] / hbm_peak
+        if kname == "window_out":
+            entry["algorithmic_GBps"] = 8.0 * m2 * n_probes / (ms / inst_steps * 1e-3) / 1e9
+            entry["frac_of_hbm_peak"] = entry["algorithmic_GBps"] / hbm_peak
+            flops2 = n_probes * m2 * 10.0 * np.log2(m2)                   # nominal 2-D FFT flops of the windows
+            entry["fp32_TFLOPs_nominal"] = flops2 / (ms / inst_steps * 1e-3) / 1e12
         kernels[kname] = entry
     top = max(kernels, key=lambda n: kernels[n]["ms_per_step"])
     if top in per_step_bytes:
