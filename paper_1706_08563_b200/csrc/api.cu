@@ -676,8 +676,51 @@ static void layout_potential(Arena& a, const prism_params* p, int n_luts, int lu
     L.cell_start = a.take<int>(cells + 1);
     L.lut_v = a.take<float>((size_t)std::max(1, n_luts) * std::max(2, lut_n));
     L.lut_rcut = a.take<double>(std::max(1, n_luts));
-    L.stage = p->potential_on_host ? a.take<float>((size_t)POT_CHUNK_SLICES * p->nx * p->ny) : nullptr;
+    L.stage = p->potential_on_host ? a.take<float>((size_t)2 * POT_CHUNK_SLICES * p->nx * p->ny) : nullptr;   // two alternating chunks
 }
+
+// Results that leave for page-locked host memory while the next piece is computed: two alternating device buffers and
+// a private copy stream.  acquire(i): the main stream may overwrite buffer i; send(i, ...): buffer i has just been
+// filled on the main stream and is copied out; join(): the main stream waits for everything sent.
+struct HostCopyOut {
+    cudaStream_t stream = nullptr;
+    cudaEvent_t ready[2] = {nullptr, nullptr}, freed[2] = {nullptr, nullptr};
+    bool used[2] = {false, false};
+    int init()
+    {
+        CU(cudaStreamCreateWithFlags(&stream, cudaStreamNonBlocking));
+        for (int i = 0; i < 2; ++i) {
+            CU(cudaEventCreateWithFlags(&ready[i], cudaEventDisableTiming));
+            CU(cudaEventCreateWithFlags(&freed[i], cudaEventDisableTiming));
+        }
+        return PRISM_OK;
+    }
+    int acquire(int i, cudaStream_t st)
+    {
+        if (used[i]) CU(cudaStreamWaitEvent(st, freed[i], 0));
+        return PRISM_OK;
+    }
+    int send(int i, void* dst, const void* src, size_t bytes, cudaStream_t st)
+    {
+        CU(cudaEventRecord(ready[i], st));
+        CU(cudaStreamWaitEvent(stream, ready[i], 0));
+        CU(cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, stream));
+        CU(cudaEventRecord(freed[i], stream));
+        used[i] = true;
+        return PRISM_OK;
+    }
+    int join(cudaStream_t st)
+    {
+        for (int i = 0; i < 2; ++i)
+            if (used[i]) CU(cudaStreamWaitEvent(st, freed[i], 0));
+        return PRISM_OK;
+    }
+    ~HostCopyOut()
+    {
+        for (int i = 0; i < 2; ++i) { if (ready[i]) cudaEventDestroy(ready[i]); if (freed[i]) cudaEventDestroy(freed[i]); }
+        if (stream) cudaStreamDestroy(stream);
+    }
+};
 
 static bool pointer_is_device(const void* ptr)
 {
@@ -899,12 +942,20 @@ int prism_build_potential(const prism_params* p, const double* atoms_xyz, const 
             LAUNCH(K_POTENTIAL, launch_potential(g, st), st);
         }
     } else {
-        for (int s0 = 0; s0 < ns; s0 += POT_CHUNK_SLICES) {
-            g.slice0 = s0; g.n_slices_chunk = std::min(POT_CHUNK_SLICES, ns - s0); g.v_out = L.stage;
+        // chunks of slices are built in one of two staging buffers and leave over a private copy stream while the
+        // next chunk is built
+        HostCopyOut out;
+        if ((rc = out.init())) return rc;
+        int n_chunk = 0;
+        for (int s0 = 0; s0 < ns; s0 += POT_CHUNK_SLICES, ++n_chunk) {
+            const int b = n_chunk % 2;
+            float* stage = L.stage + (size_t)b * POT_CHUNK_SLICES * npix;
+            g.slice0 = s0; g.n_slices_chunk = std::min(POT_CHUNK_SLICES, ns - s0); g.v_out = stage;
+            if ((rc = out.acquire(b, st))) return rc;
             LAUNCH(K_POTENTIAL, launch_potential(g, st), st);
-            CU(cudaMemcpyAsync(v + (size_t)s0 * npix, L.stage, (size_t)g.n_slices_chunk * npix * sizeof(float),
-                               cudaMemcpyDeviceToHost, st));
+            if ((rc = out.send(b, v + (size_t)s0 * npix, stage, (size_t)g.n_slices_chunk * npix * sizeof(float), st))) return rc;
         }
+        if ((rc = out.join(st))) return rc;
     }
     return PRISM_OK;
 }
@@ -949,37 +1000,10 @@ int prism_compute_smatrix(const prism_params* p, const float* v, int32_t* beams_
     const bool blocked = blocked_grid(p->nx, p->ny);
     // S in host memory: finished layers leave over a private copy stream from one of two alternating
     // buffers (wave batches, or ROW_FINAL staging chunks on blocked grids) while the next batch / chunk is computed
-    struct CopyOut {
-        cudaStream_t stream = nullptr;
-        cudaEvent_t ready[2] = {nullptr, nullptr}, freed[2] = {nullptr, nullptr};
-        bool used[2] = {false, false};
-        ~CopyOut()
-        {
-            for (int i = 0; i < 2; ++i) { if (ready[i]) cudaEventDestroy(ready[i]); if (freed[i]) cudaEventDestroy(freed[i]); }
-            if (stream) cudaStreamDestroy(stream);
-        }
-    } out;
-    if (s_on_host) {
-        cudaError_t ce = cudaStreamCreateWithFlags(&out.stream, cudaStreamNonBlocking);
-        for (int i = 0; i < 2 && ce == cudaSuccess; ++i) {
-            ce = cudaEventCreateWithFlags(&out.ready[i], cudaEventDisableTiming);
-            if (ce == cudaSuccess) ce = cudaEventCreateWithFlags(&out.freed[i], cudaEventDisableTiming);
-        }
-        if (ce != cudaSuccess) { feed.release(); return cuda_fail(ce, "copy-out stream"); }
-    }
-    // buffer i is about to be overwritten on the main stream / has just been filled and may leave
-    auto acquire = [&](int i) -> int {
-        if (out.used[i]) CU(cudaStreamWaitEvent(st, out.freed[i], 0));
-        return PRISM_OK;
-    };
-    auto send = [&](int i, void* dst, const void* src, size_t bytes) -> int {
-        CU(cudaEventRecord(out.ready[i], st));
-        CU(cudaStreamWaitEvent(out.stream, out.ready[i], 0));
-        CU(cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, out.stream));
-        CU(cudaEventRecord(out.freed[i], out.stream));
-        out.used[i] = true;
-        return PRISM_OK;
-    };
+    HostCopyOut out;
+    if (s_on_host && (rc = out.init())) { feed.release(); return rc; }
+    auto acquire = [&](int i) -> int { return out.acquire(i, st); };
+    auto send = [&](int i, void* dst, const void* src, size_t bytes) -> int { return out.send(i, dst, src, bytes, st); };
     auto run = [&]() -> int {
         int n_batch = 0, n_chunk = 0;
         for (int b0 = 0; b0 < n_beams; b0 += batch, ++n_batch) {
@@ -1036,9 +1060,7 @@ int prism_compute_smatrix(const prism_params* p, const float* v, int32_t* beams_
             }
         }
         // the call's work is complete on `st` only when the last layers have left
-        for (int i = 0; i < 2; ++i)
-            if (out.used[i]) CU(cudaStreamWaitEvent(st, out.freed[i], 0));
-        return PRISM_OK;
+        return out.join(st);
     };
     rc = run();
     feed.release();
