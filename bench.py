@@ -527,6 +527,10 @@ def run_prism(name, steps, warmup, world, rank, local, dist, want_cpu_baseline, 
                               "fp32_frac": flops / (slice_ms * 1e-3) / 1e12 / FP32_PEAK_TFLOPS}
     roofline["measured_in"] = (f"instrumented pass of {inst_steps} step(s) after the timed region (CUDA events around "
                                "every launch on the launching stream)")
+    if w.nx == 2048 and w.ny == 2048:
+        roofline["note"] = ("the two 2048-point passes take the same time; the row pass is FP32-bound (ncu: "
+                            "sm__pipe_fma_cycles_active 72 %, DRAM 51 %), the column pass waits on its tile and its stores "
+                            "(FMA pipe 52 %): profiles/r02_p16.md sections 3a, 3b")
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": warmup,
