@@ -99,39 +99,14 @@ template <> struct Dft<8> {
     }
 };
 
-template <> struct Dft<16> {
-    __device__ __forceinline__ static void run(C2* a)
-    {
-        const float c1 = 0.92387953251128675613f, s1 = 0.38268343236508977173f;   // cos, sin(pi/8)
-        const float h  = 0.70710678118654752440f;
-        C2 y[4][4];
-#pragma unroll
-        for (int n2 = 0; n2 < 4; ++n2) {
-            y[n2][0] = a[n2]; y[n2][1] = a[n2 + 4]; y[n2][2] = a[n2 + 8]; y[n2][3] = a[n2 + 12];
-            Dft<4>::run(y[n2]);
-        }
-        // w16^m = exp(-2 pi i m / 16)
-        y[1][1] = cmulc(y[1][1], c1, -s1);
-        y[1][2] = cmulc(y[1][2], h, -h);
-        y[1][3] = cmulc(y[1][3], s1, -c1);
-        y[2][1] = cmulc(y[2][1], h, -h);
-        y[2][2] = { y[2][2].y, neg2(y[2][2].x) };
-        y[2][3] = cmulc(y[2][3], -h, -h);
-        y[3][1] = cmulc(y[3][1], s1, -c1);
-        y[3][2] = cmulc(y[3][2], -h, -h);
-        y[3][3] = cmulc(y[3][3], -c1, s1);
-#pragma unroll
-        for (int k1 = 0; k1 < 4; ++k1) {
-            C2 z[4] = { y[0][k1], y[1][k1], y[2][k1], y[3][k1] };
-            Dft<4>::run(z);
-            a[k1] = z[0]; a[k1 + 4] = z[1]; a[k1 + 8] = z[2]; a[k1 + 12] = z[3];
-        }
-    }
-};
-
-// Twiddle w32^m = (-i)^q * cos(t) * (1 - i tan(t)) with q the nearest quarter turn and |t| <= pi/4, t = 2 pi j / 32.
-__device__ __forceinline__ constexpr int tw_q(int m) { return (m % 8 == 4) ? m / 8 : (m + 4) / 8; }
-__device__ __forceinline__ constexpr int tw_j(int m) { return m - 8 * tw_q(m); }
+// ---- radix-4 butterfly over twiddled inputs, scaled-twiddle form (both lanes) ---------------------------------
+// out = DFT4(z0, y1 w^k1, y2 w^(2 k1), y3 w^(3 k1)), w = exp(-2 pi i / R), R = 16 or 32.  Each twiddle is written
+// w^m = (-i)^q cos(t) (1 - i tan(t)) with q the nearest quarter turn and |t| <= pi/4: u = (-i)^q y (1 - i tan) costs two
+// FFMA2 -- the quarter turn is a renaming -- and the cosines ride on the adds of the butterfly, which become FFMA2 at
+// the same cost:  z1 + z3 = c1 (u1 + (c3 / c1) u3),  z0 + z2 = z0 + c2 u2,  out = t0 + c1 S ...
+// 22 packed instructions instead of 28 (three complex multiplies + 16 adds).
+template <int R> __device__ __forceinline__ constexpr int tw_q(int m)
+{ return (m % (R / 4) == R / 8) ? m / (R / 4) : (m + R / 8) / (R / 4); }
 // a * (-i)^q
 __device__ __forceinline__ C2 rotq(C2 a, int q)
 {
@@ -142,10 +117,62 @@ __device__ __forceinline__ C2 rotq(C2 a, int q)
         default: return a;
     }
 }
+template <int R>
+__device__ __forceinline__ void twiddled_dft4(C2 z0, C2 y1, C2 y2, C2 y3, int k1, C2& o0, C2& o1, C2& o2, C2& o3)
+{
+    static_assert(R == 16 || R == 32, "tables");
+    // cos and tan of 2 pi j / R for j = -R/8 .. R/8
+    constexpr float C16[5] = { 0.70710678118654752440f, 0.92387953251128675613f, 1.f, 0.92387953251128675613f,
+                               0.70710678118654752440f };
+    constexpr float T16[5] = { -1.f, -0.41421356237309504880f, 0.f, 0.41421356237309504880f, 1.f };
+    constexpr float C32[9] = { 0.70710678118654752440f, 0.83146961230254523708f, 0.92387953251128675613f,
+                               0.98078528040323044913f, 1.f, 0.98078528040323044913f, 0.92387953251128675613f,
+                               0.83146961230254523708f, 0.70710678118654752440f };
+    constexpr float T32[9] = { -1.f, -0.66817863791929891999f, -0.41421356237309504880f, -0.19891236737965800691f, 0.f,
+                               0.19891236737965800691f, 0.41421356237309504880f, 0.66817863791929891999f, 1.f };
+    const C2 y[4] = { z0, y1, y2, y3 };
+    C2 u[4];
+    float c[4] = { 1.f, 1.f, 1.f, 1.f };
+#pragma unroll
+    for (int n2 = 1; n2 < 4; ++n2) {
+        const int m = n2 * k1, q = tw_q<R>(m), j = m - q * (R / 4);
+        const float tau = R == 16 ? T16[j + 2] : T32[j + 4];
+        c[n2] = R == 16 ? C16[j + 2] : C32[j + 4];
+        const C2 v = y[n2];
+        const C2 w = (j == 0) ? v : C2{ fma2(v.y, bc(tau), v.x), fma2(v.x, bc(-tau), v.y) };   // v (1 - i tan)
+        u[n2] = rotq(w, q);
+    }
+    const C2 t0 = { fma2(u[2].x, bc(c[2]), z0.x), fma2(u[2].y, bc(c[2]), z0.y) };
+    const C2 t1 = { fma2(u[2].x, bc(-c[2]), z0.x), fma2(u[2].y, bc(-c[2]), z0.y) };
+    const float r = c[3] / c[1];
+    const C2 sp = { fma2(u[3].x, bc(r), u[1].x), fma2(u[3].y, bc(r), u[1].y) };      // (z1 + z3) / c1
+    const C2 dm = { fma2(u[3].x, bc(-r), u[1].x), fma2(u[3].y, bc(-r), u[1].y) };    // (z1 - z3) / c1
+    o0 = { fma2(sp.x, bc(c[1]), t0.x), fma2(sp.y, bc(c[1]), t0.y) };
+    o2 = { fma2(sp.x, bc(-c[1]), t0.x), fma2(sp.y, bc(-c[1]), t0.y) };
+    o1 = { fma2(dm.y, bc(c[1]), t1.x), fma2(dm.x, bc(-c[1]), t1.y) };                // t1 + (-i) c1 dm
+    o3 = { fma2(dm.y, bc(-c[1]), t1.x), fma2(dm.x, bc(c[1]), t1.y) };
+}
 
-#ifndef PRISM_PK_TAN_TWIDDLES
-#define PRISM_PK_TAN_TWIDDLES 1
-#endif
+template <> struct Dft<16> {
+    __device__ __forceinline__ static void run(C2* a)
+    {
+        // n = 4 n1 + n2 ; k = k1 + 4 k2.  Y[n2][k1] = DFT4 over n1, then twiddle w16^(n2 k1), DFT4 over n2.
+        C2 y[4][4];
+#pragma unroll
+        for (int n2 = 0; n2 < 4; ++n2) {
+            y[n2][0] = a[n2]; y[n2][1] = a[n2 + 4]; y[n2][2] = a[n2 + 8]; y[n2][3] = a[n2 + 12];
+            Dft<4>::run(y[n2]);
+        }
+        {
+            C2 z[4] = { y[0][0], y[1][0], y[2][0], y[3][0] };
+            Dft<4>::run(z);
+            a[0] = z[0]; a[4] = z[1]; a[8] = z[2]; a[12] = z[3];
+        }
+#pragma unroll
+        for (int k1 = 1; k1 < 4; ++k1)
+            twiddled_dft4<16>(y[0][k1], y[1][k1], y[2][k1], y[3][k1], k1, a[k1], a[k1 + 4], a[k1 + 8], a[k1 + 12]);
+    }
+};
 
 template <> struct Dft<32> {
     __device__ __forceinline__ static void run(C2* a)
@@ -158,75 +185,14 @@ template <> struct Dft<32> {
             for (int n1 = 0; n1 < 8; ++n1) y[n2][n1] = a[4 * n1 + n2];
             Dft<8>::run(y[n2]);
         }
-#if PRISM_PK_TAN_TWIDDLES
-        // Scaled twiddles: y w = (-i)^q c (y (1 - i tan)) costs two FFMA2 for u = (-i)^q y (1 - i tan) -- the quarter
-        // turn is a renaming -- and the cosines ride on the adds of the radix-4 butterfly, which become FFMA2 at the
-        // same cost:  z1 + z3 = c1 (u1 + (c3 / c1) u3),  z0 + z2 = z0 + c2 u2,  out = t0 + c1 S ...
-        // 22 packed instructions per column k1 instead of 28 (three complex multiplies + 16 adds).
-        constexpr float CJ[9] = { 0.70710678118654752440f, 0.83146961230254523708f, 0.92387953251128675613f,
-                                  0.98078528040323044913f, 1.f, 0.98078528040323044913f, 0.92387953251128675613f,
-                                  0.83146961230254523708f, 0.70710678118654752440f };                 // cos(2 pi j / 32), j = -4 .. 4
-        constexpr float TJ[9] = { -1.f, -0.66817863791929891999f, -0.41421356237309504880f, -0.19891236737965800691f, 0.f,
-                                  0.19891236737965800691f, 0.41421356237309504880f, 0.66817863791929891999f, 1.f };   // tan
         {
             C2 z[4] = { y[0][0], y[1][0], y[2][0], y[3][0] };
             Dft<4>::run(z);
             a[0] = z[0]; a[8] = z[1]; a[16] = z[2]; a[24] = z[3];
         }
 #pragma unroll
-        for (int k1 = 1; k1 < 8; ++k1) {
-            C2 u[4];
-            float c[4] = { 1.f, 1.f, 1.f, 1.f };
-#pragma unroll
-            for (int n2 = 1; n2 < 4; ++n2) {
-                const int m = n2 * k1, j = tw_j(m);
-                const float tau = TJ[j + 4];
-                c[n2] = CJ[j + 4];
-                const C2 v = y[n2][k1];
-                const C2 w = (j == 0) ? v : C2{ fma2(v.y, bc(tau), v.x), fma2(v.x, bc(-tau), v.y) };   // v (1 - i tan)
-                u[n2] = rotq(w, tw_q(m));
-            }
-            const C2 z0 = y[0][k1];
-            const C2 t0 = { fma2(u[2].x, bc(c[2]), z0.x), fma2(u[2].y, bc(c[2]), z0.y) };
-            const C2 t1 = { fma2(u[2].x, bc(-c[2]), z0.x), fma2(u[2].y, bc(-c[2]), z0.y) };
-            const float r = c[3] / c[1];
-            const C2 sp = { fma2(u[3].x, bc(r), u[1].x), fma2(u[3].y, bc(r), u[1].y) };      // (z1 + z3) / c1
-            const C2 dm = { fma2(u[3].x, bc(-r), u[1].x), fma2(u[3].y, bc(-r), u[1].y) };    // (z1 - z3) / c1
-            a[k1]      = { fma2(sp.x, bc(c[1]), t0.x), fma2(sp.y, bc(c[1]), t0.y) };
-            a[k1 + 16] = { fma2(sp.x, bc(-c[1]), t0.x), fma2(sp.y, bc(-c[1]), t0.y) };
-            a[k1 + 8]  = { fma2(dm.y, bc(c[1]), t1.x), fma2(dm.x, bc(-c[1]), t1.y) };       // t1 + (-i) c1 dm
-            a[k1 + 24] = { fma2(dm.y, bc(-c[1]), t1.x), fma2(dm.x, bc(c[1]), t1.y) };
-        }
-#else
-        // w32^m = exp(-2 pi i m / 32) = (WC[m], -WS[m]) for m <= 21
-        constexpr float WC[22] = { 1.f, 0.98078528040323044913f, 0.92387953251128675613f, 0.83146961230254523708f,
-                                   0.70710678118654752440f, 0.55557023301960222474f, 0.38268343236508977173f,
-                                   0.19509032201612826785f, 0.f, -0.19509032201612826785f, -0.38268343236508977173f,
-                                   -0.55557023301960222474f, -0.70710678118654752440f, -0.83146961230254523708f,
-                                   -0.92387953251128675613f, -0.98078528040323044913f, -1.f, -0.98078528040323044913f,
-                                   -0.92387953251128675613f, -0.83146961230254523708f, -0.70710678118654752440f,
-                                   -0.55557023301960222474f };
-        constexpr float WS[22] = { 0.f, 0.19509032201612826785f, 0.38268343236508977173f, 0.55557023301960222474f,
-                                   0.70710678118654752440f, 0.83146961230254523708f, 0.92387953251128675613f,
-                                   0.98078528040323044913f, 1.f, 0.98078528040323044913f, 0.92387953251128675613f,
-                                   0.83146961230254523708f, 0.70710678118654752440f, 0.55557023301960222474f,
-                                   0.38268343236508977173f, 0.19509032201612826785f, 0.f, -0.19509032201612826785f,
-                                   -0.38268343236508977173f, -0.55557023301960222474f, -0.70710678118654752440f,
-                                   -0.83146961230254523708f };
-#pragma unroll
-        for (int n2 = 1; n2 < 4; ++n2)
-#pragma unroll
-            for (int k1 = 1; k1 < 8; ++k1) {
-                if (n2 * k1 == 8) y[n2][k1] = { y[n2][k1].y, neg2(y[n2][k1].x) };      // * (-i)
-                else y[n2][k1] = cmulc(y[n2][k1], WC[n2 * k1], -WS[n2 * k1]);
-            }
-#pragma unroll
-        for (int k1 = 0; k1 < 8; ++k1) {
-            C2 z[4] = { y[0][k1], y[1][k1], y[2][k1], y[3][k1] };
-            Dft<4>::run(z);
-            a[k1] = z[0]; a[k1 + 8] = z[1]; a[k1 + 16] = z[2]; a[k1 + 24] = z[3];
-        }
-#endif
+        for (int k1 = 1; k1 < 8; ++k1)
+            twiddled_dft4<32>(y[0][k1], y[1][k1], y[2][k1], y[3][k1], k1, a[k1], a[k1 + 8], a[k1 + 16], a[k1 + 24]);
     }
 };
 
