@@ -236,6 +236,16 @@ def test_large_grid_parity(G, name):
     rows = np.array([0, 5, len(xy) - 1])
     ref2 = O.prism_probes(p, s.cpu().numpy().astype(np.complex128), beams, xy[rows])
     assert rel_l2(out[rows], ref2) < 2e-5
+    if name == "T2048f16":
+        # S-matrix in page-locked host memory on the blocked layout (ROW_FINAL staging chunks leave over the copy
+        # stream, several beam batches): bit-identical to the resident path
+        from paper_1706_08563_b200 import prism
+        ph = prism.params_from_workload(w, smatrix_on_host=1, batch=5)
+        s_host = torch.empty_like(s, device="cpu").pin_memory()
+        b2 = prism.compute_smatrix(ph, v, s_host, G.ws(ph, prism.WS_SMATRIX))
+        torch.cuda.synchronize()
+        assert np.array_equal(beams, b2) and torch.equal(s_host, s.cpu())
+        del s_host
     del s
     ms = G.gpu_multislice(w, v)
     ref3 = O.multislice_probes(p, v_ref, xy[rows])
