@@ -106,8 +106,10 @@ template <int Q> struct LatticeCfg {
     static constexpr size_t SMEM = (size_t)TP * PS * sizeof(float2);
 };
 
-template <int Q>
-__global__ void __launch_bounds__(LatticeCfg<Q>::NT, 512 / LatticeCfg<Q>::NT) lattice_dft_kernel(LatticeArgs g)
+// MULTI: more than one beam folds onto some residue (n_slots > 1); a separate instantiation, so that its batched loads
+// do not cost the single-slot kernel a resident CTA (92 against 80 registers)
+template <int Q, bool MULTI>
+__global__ void __launch_bounds__(LatticeCfg<Q>::NT, MULTI ? 2 : 3) lattice_dft_kernel(LatticeArgs g)
 {
     using C = LatticeCfg<Q>;
     constexpr int TP = C::TP, RS = C::RS, PS = C::PS, CPI = C::NT / TP;   // cells per iteration
@@ -125,7 +127,7 @@ __global__ void __launch_bounds__(LatticeCfg<Q>::NT, 512 / LatticeCfg<Q>::NT) la
         const size_t layer = g.slab ? (size_t)g.nx * g.slab_cap : (size_t)g.nx * g.ny;
         const float2* src = g.s + (size_t)(g.slab ? (g.slab_u0 + r) % g.slab_cap : y) * g.nx + xt + px;
         float2* dst = sm + px * PS;
-        if (g.n_slots == 1) {
+        if (!MULTI) {
 #pragma unroll 16
             for (int c = c0; c < Q * Q; c += CPI) {
                 const int b = __ldg(g.cell_beam + c);
@@ -134,15 +136,19 @@ __global__ void __launch_bounds__(LatticeCfg<Q>::NT, 512 / LatticeCfg<Q>::NT) la
                 dst[(c / Q) * RS + (c % Q)] = r;
             }
         } else {
-#pragma unroll 2
+#pragma unroll 4
             for (int c = c0; c < Q * Q; c += CPI) {
-                float2 acc = make_float2(0.f, 0.f);
-                for (int sl = 0; sl < g.n_slots; ++sl) {
-                    const int b = __ldg(g.cell_beam + sl * Q * Q + c);
-                    const float2 a = b >= 0 ? __ldg(g.coef + b) : make_float2(0.f, 0.f);
-                    const float2 v = __ldg(src + (size_t)max(b, 0) * layer);
-                    acc = cadd(acc, cmul(a, v));
+                // up to four beams fold onto a residue; the loads of a residue's slots are independent (issued together)
+                float2 val[4], cf[4];
+#pragma unroll
+                for (int sl = 0; sl < 4; ++sl) {
+                    const int b = sl < g.n_slots ? __ldg(g.cell_beam + sl * Q * Q + c) : -1;
+                    cf[sl] = b >= 0 ? __ldg(g.coef + b) : make_float2(0.f, 0.f);
+                    val[sl] = b >= 0 ? __ldg(src + (size_t)b * layer) : make_float2(0.f, 0.f);      // empty slot: no load
                 }
+                float2 acc = make_float2(0.f, 0.f);
+#pragma unroll
+                for (int sl = 0; sl < 4; ++sl) acc = cadd(acc, cmul(cf[sl], val[sl]));
                 dst[(c / Q) * RS + (c % Q)] = acc;
             }
         }
@@ -200,12 +206,15 @@ static cudaError_t launch_lattice_q(const LatticeArgs& g, cudaStream_t stream)
 {
     using C = LatticeCfg<Q>;
     static PerDevice once{};
-    if (cudaError_t e = opt_in_smem(lattice_dft_kernel<Q>, C::SMEM, once); e != cudaSuccess) return e;
+    if (cudaError_t e = opt_in_smem(lattice_dft_kernel<Q, false>, C::SMEM, once); e != cudaSuccess) return e;
+    static PerDevice once_multi{};
+    if (cudaError_t e = opt_in_smem(lattice_dft_kernel<Q, true>, C::SMEM, once_multi); e != cudaSuccess) return e;
     if (g.nx % C::TP) return cudaErrorInvalidValue;
     const long long blocks = (long long)(g.nx / C::TP) * g.n_pix_rows;
     if (blocks <= 0) return cudaSuccess;
     if (blocks > 0x7fffffffLL) return cudaErrorInvalidValue;
-    lattice_dft_kernel<Q><<<(unsigned)blocks, C::NT, C::SMEM, stream>>>(g);
+    if (g.n_slots > 1) lattice_dft_kernel<Q, true><<<(unsigned)blocks, C::NT, C::SMEM, stream>>>(g);
+    else lattice_dft_kernel<Q, false><<<(unsigned)blocks, C::NT, C::SMEM, stream>>>(g);
     return cudaGetLastError();
 }
 
