@@ -446,7 +446,7 @@ def run_prism(name, steps, warmup, world, rank, local, dist, want_cpu_baseline, 
     # 8 x 8 sub-grid of the probe positions
     ms_n = 64 if name == "P16" else max(1, min(8, w.probes_x, w.probes_y))
     w_ms = w.with_(probes_x=ms_n, probes_y=ms_n, probe_step=(w.cell[0] / ms_n, w.cell[1] / ms_n),
-                   batch=256 if name == "P16" else w.batch)
+                   batch=1024 if name == "P16" else w.batch)   # P16: 4 sweeps of the streamed potential
     p_ms = prism.params_from_workload(w_ms)
     del ws
     torch.cuda.empty_cache()
