@@ -132,6 +132,30 @@ int prism_build_potential(const prism_params* p, const double* atoms_xyz, const 
                           int64_t n_atoms, const prism_lut* luts, int32_t n_luts, float* v,
                           void* workspace, size_t workspace_bytes, void* cuda_stream);
 
+/* prism_build_potential for callers that cannot give it a workspace because they may not allocate device memory:
+ * code running inside a host application whose own pool owns the device (no cudaMalloc of its own allowed), a
+ * process that has already handed all device memory to another library, or a caller inside a phase in which the
+ * CUDA allocator must not be entered.  Same arguments, same kernel, same result (bit for bit) as
+ * prism_build_potential, minus `workspace`: the scratch the kernel reads (sorted atoms, cell starts, radial
+ * tables) is a fixed array of PRISM_STATIC_SCRATCH_BYTES inside the library image.  Every GPU that loads the
+ * library carries those bytes from load until the process exits, whether this call is used or not.
+ *   Limit: prism_workspace_bytes(p, PRISM_WS_POTENTIAL) + 32 * n_atoms + 512 <= PRISM_STATIC_SCRATCH_BYTES
+ *   (configs 1-4 of BASELINE.json fit; config 5's 400 x 2048^2 cell table does not) and potential_on_host = 0
+ *   (v is device memory).  Anything beyond returns PRISM_EUNSUPPORTED, with the byte counts in
+ *   prism_last_error(); nothing is launched.
+ *   The call enters no allocator: no cudaMalloc / cudaFree, no stream or event creation (keep prism_timing_enable
+ *   off, which creates events).  Host-side tables are ordinary host memory, as in prism_build_potential.
+ *   The first call on each device looks the array's device address up (cudaGetSymbolAddress, with that device
+ *   current); make that first call outside any stream capture.
+ *   All calls on a device share the one array, and it keeps what the last call left in it.  Every byte the
+ *   kernel reads is uploaded on `cuda_stream` by the same call before its launch, so nothing relies on earlier
+ *   contents and nothing needs clearing -- but two calls whose GPU work overlaps (different streams or threads,
+ *   same device) race on it.  Order them on one stream, or with events. */
+#define PRISM_STATIC_SCRATCH_BYTES ((size_t)8 << 20)
+int prism_build_potential_static(const prism_params* p, const double* atoms_xyz, const int32_t* z_number,
+                                 int64_t n_atoms, const prism_lut* luts, int32_t n_luts, float* v,
+                                 void* cuda_stream);
+
 /* Compact S-matrix (Fig. 1g-h): every beam's plane wave exp(+2 pi i q_b . r) is taken
  * through all slices, psi <- IFFT2[ P . FFT2[ psi . exp(i sigma V_s) ] ] (Eq. 1, Eq. 2 with the 2/3
  * band-limit on P), and its real-space exit wave stored as layer b at full resolution (R17).

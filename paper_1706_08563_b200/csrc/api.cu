@@ -961,6 +961,37 @@ int prism_build_potential(const prism_params* p, const double* atoms_xyz, const 
 }
 
 // ---------------------------------------------------------------------------------------------------------
+// The same call on the library's built-in scratch array (potential.cu) instead of a caller workspace: for callers
+// that may not allocate device memory.  Nothing here allocates on the device; the size is checked first so that an
+// oversized request fails with the numbers in prism_last_error() instead of a bare PRISM_ENOMEM.
+static_assert(PRISM_STATIC_SCRATCH_BYTES == POT_STATIC_BYTES, "prism.h and potential.cu disagree on the scratch size");
+int prism_build_potential_static(const prism_params* p, const double* atoms_xyz, const int32_t* z_number,
+                                 int64_t n_atoms, const prism_lut* luts, int32_t n_luts, float* v,
+                                 void* cuda_stream)
+{
+    int rc = check_common(p);
+    if (rc) return rc;
+    if (n_atoms < 0) return PRISM_EINVAL;
+    if (p->potential_on_host) {
+        snprintf(g_last_error, sizeof(g_last_error),
+                 "prism_build_potential_static: potential_on_host needs staging buffers and a copy stream; v must be device memory");
+        return PRISM_EUNSUPPORTED;
+    }
+    const size_t fixed = prism_workspace_bytes(p, PRISM_WS_POTENTIAL);
+    const size_t atoms = (size_t)std::min<int64_t>(n_atoms, (int64_t)PRISM_STATIC_SCRATCH_BYTES);     // beyond that it cannot fit anyway
+    const size_t need = fixed + 512 + atoms * sizeof(PotAtom);
+    if (fixed == 0 || need > PRISM_STATIC_SCRATCH_BYTES) {
+        snprintf(g_last_error, sizeof(g_last_error),
+                 "prism_build_potential_static: %zu bytes of scratch needed (%lld atoms, %d slices of %d x %d), the built-in array holds %zu",
+                 need, (long long)n_atoms, p->n_slices, p->nx, p->ny, (size_t)PRISM_STATIC_SCRATCH_BYTES);
+        return PRISM_EUNSUPPORTED;
+    }
+    void* scratch = nullptr;
+    CU(potential_static_scratch(&scratch));        // device address of the array on the current device, not its host-side name
+    return prism_build_potential(p, atoms_xyz, z_number, n_atoms, luts, n_luts, v, scratch, POT_STATIC_BYTES, cuda_stream);
+}
+
+// ---------------------------------------------------------------------------------------------------------
 int prism_compute_smatrix(const prism_params* p, const float* v, int32_t* beams_out, void* s,
                           void* workspace, size_t workspace_bytes, void* cuda_stream)
 {

@@ -12,6 +12,8 @@
 // r_cut, in the fixed sorted order.  No atomics, no memset, one coalesced write per
 // pixel, and a bit-reproducible result.  Distances and the cut decision are taken
 // in fp64 (the table interpolation too); the sum is rounded once to fp32.
+#include <mutex>
+
 #include "prism_internal.h"
 
 namespace prism {
@@ -65,6 +67,39 @@ cudaError_t launch_potential(const PotentialArgs& g, cudaStream_t stream)
     dim3 grid((unsigned)(g.tiles_x * g.tiles_y), (unsigned)g.n_slices_chunk);
     potential_kernel<<<grid, g.tile * g.tile, 0, stream>>>(g);
     return cudaGetLastError();
+}
+
+// ---- scratch for prism_build_potential_static -----------------------------------------------------------
+// Some hosts of this library may not allocate device memory themselves: a plug-in that runs inside someone
+// else's allocator (a framework whose memory pool owns the whole device), a process that has handed every byte
+// to another library, or code running between the capture calls of a stream where cudaMalloc is illegal.  For
+// them the kernel's scratch (sorted atoms, cell starts, radial tables) lives here, inside the library image:
+// every device that loads the library holds these POT_STATIC_BYTES from load until process exit.
+//
+// Host code must never hand `pot_static_scratch` itself to a kernel: in host code that name is the host-side
+// shadow of the symbol, not a device address.  The device address is looked up once per device with
+// cudaGetSymbolAddress (below), with that device current, and cached.
+static __device__ __align__(256) unsigned char pot_static_scratch[POT_STATIC_BYTES];
+
+cudaError_t potential_static_scratch(void** ptr)
+{
+    constexpr int MAX_DEVICES = 64;
+    static std::mutex mu;
+    static void* address[MAX_DEVICES] = {};
+    *ptr = nullptr;
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= MAX_DEVICES) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(mu);
+    if (!address[dev]) {
+        void* p = nullptr;
+        e = cudaGetSymbolAddress(&p, pot_static_scratch);       // this device's copy of the array
+        if (e != cudaSuccess) return e;
+        address[dev] = p;
+    }
+    *ptr = address[dev];
+    return cudaSuccess;
 }
 
 }  // namespace prism

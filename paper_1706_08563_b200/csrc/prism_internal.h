@@ -224,5 +224,9 @@ struct PotentialArgs {
     float*         v_out;       // [n_slices_chunk][ny][nx]
 };
 cudaError_t launch_potential(const PotentialArgs& args, cudaStream_t stream);
+// Device address, on the current device, of the library's built-in scratch array of POT_STATIC_BYTES bytes
+// (prism_build_potential_static).  The first call on a device looks the address up; no allocation.
+constexpr size_t POT_STATIC_BYTES = (size_t)8 << 20;
+cudaError_t potential_static_scratch(void** ptr);
 
 }  // namespace prism

@@ -20,7 +20,7 @@ PRISM_OK, PRISM_EINVAL, PRISM_ENOMEM, PRISM_ECUDA, PRISM_EUNSUPPORTED, PRISM_ENO
 WS_SMATRIX, WS_OUTPUT, WS_MULTISLICE, WS_POTENTIAL = 0, 1, 2, 3
 
 EXPORTS = ["prism_workspace_bytes", "prism_num_bins", "prism_num_beams", "prism_band_columns", "prism_constants",
-           "prism_build_potential", "prism_compute_smatrix", "prism_compute_output",
+           "prism_build_potential", "prism_build_potential_static", "prism_compute_smatrix", "prism_compute_output",
            "multislice_compute_output", "prism_compute_patterns", "multislice_compute_patterns",
            "prism_compute_detectors", "multislice_compute_detectors", "prism_accumulate", "prism_strerror", "prism_last_error", "prism_launch_count",
            "prism_timing_enable", "prism_timing_classes", "prism_timing_class_name", "prism_timing_read"]
@@ -77,6 +77,8 @@ def _load() -> C.CDLL:
     lib.prism_constants.argtypes = [C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_double)]
     lib.prism_build_potential.restype = C.c_int
     lib.prism_build_potential.argtypes = [pp, vp, vp, i64, C.POINTER(Lut), i32, vp, vp, sz, vp]
+    lib.prism_build_potential_static.restype = C.c_int
+    lib.prism_build_potential_static.argtypes = [pp, vp, vp, i64, C.POINTER(Lut), i32, vp, vp]
     lib.prism_compute_smatrix.restype = C.c_int
     lib.prism_compute_smatrix.argtypes = [pp, vp, vp, vp, vp, sz, vp]
     lib.prism_compute_output.restype = C.c_int
@@ -206,6 +208,32 @@ def build_potential(p: Params, atoms_xyz, z_number, lut_z, r_cut, lut_v, v_out, 
     _check(_lib.prism_build_potential(C.byref(p), atoms.ctypes.data, zn.ctypes.data, len(zn), luts, len(lut_z),
                                       _ptr(v_out), _ptr(workspace), workspace.numel() * workspace.element_size(),
                                       _stream_ptr(stream)), "prism_build_potential")
+    return v_out
+
+
+STATIC_SCRATCH_BYTES = 8 << 20       # PRISM_STATIC_SCRATCH_BYTES of include/prism.h
+
+
+def build_potential_static(p: Params, atoms_xyz, z_number, lut_z, r_cut, lut_v, v_out, stream=None):
+    """``prism_build_potential_static``: ``build_potential`` without a workspace, for callers that may not
+    allocate device memory (they run inside another program's memory pool, or all of the device is already
+    spoken for).  The kernel's scratch is an 8 MiB array built into the library, shared by every call on the
+    device; requests that need more raise ``PrismError`` (``PRISM_EUNSUPPORTED``) with the byte counts.
+    ``v_out`` must be a CUDA tensor.  Same result as ``build_potential``, bit for bit."""
+    atoms = np.ascontiguousarray(atoms_xyz, dtype=np.float64).reshape(-1, 3)
+    zn = np.ascontiguousarray(z_number, dtype=np.int32)
+    tabs = np.ascontiguousarray(lut_v, dtype=np.float32).reshape(len(lut_z), -1 if len(lut_z) else 0)
+    luts = (Lut * len(lut_z))()
+    for i, z in enumerate(lut_z):
+        luts[i].z, luts[i].n, luts[i].r_cut = int(z), tabs.shape[1], float(r_cut)
+        luts[i].v = tabs[i].ctypes.data_as(C.POINTER(C.c_float))
+    code = _lib.prism_build_potential_static(C.byref(p), atoms.ctypes.data, zn.ctypes.data, len(zn), luts,
+                                             len(lut_z), _ptr(v_out), _stream_ptr(stream))
+    if code == PRISM_EUNSUPPORTED:
+        err = PrismError(code, "prism_build_potential_static")
+        err.args = (f"{err.args[0]}: {_lib.prism_last_error().decode()}",)
+        raise err
+    _check(code, "prism_build_potential_static")
     return v_out
 
 
