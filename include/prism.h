@@ -47,7 +47,7 @@ enum {
     PRISM_EINVAL       = -1,  /* null pointer, unsupported grid, f does not divide n, alpha beyond the band-limit, ... */
     PRISM_ENOMEM       = -2,  /* workspace too small (ask prism_workspace_bytes)                                      */
     PRISM_ECUDA        = -3,  /* a CUDA call failed; prism_last_error() holds the CUDA message                        */
-    PRISM_EUNSUPPORTED = -4,  /* valid request outside what this build covers (e.g. window larger than 128 x 128)    */
+    PRISM_EUNSUPPORTED = -4,  /* valid request outside what this build covers (e.g. a window side above 128 points)   */
     PRISM_ENOLUT       = -5   /* an atom's Z has no lookup table                                                     */
 };
 
@@ -72,7 +72,8 @@ typedef struct prism_params {
     double  voltage;            /* -> lambda, sigma (relativistic closed forms, fp64; R0)                   */
     double  alpha;              /* probe semi-angle; hard aperture edge, '<=' (R4)                          */
     double  defocus, cs;        /* C1, C3: chi(q) = pi lambda q^2 C1 + (pi/2) C3 lambda^3 q^4, probe carries exp(-i chi) (R5) */
-    int32_t f;                  /* PRISM interpolation factor; must divide nx and ny; window = n / f (R8)    */
+    int32_t f;                  /* PRISM interpolation factor; must divide nx and ny; window = n / f (R8);
+                                   this build: 16 <= nx / f <= 128 and 16 <= ny / f <= 128, else PRISM_EUNSUPPORTED */
     int32_t probes_x, probes_y; /* probe grid; probe (ix, iy) sits at origin + (ix, iy) * step (R10)         */
     double  probe_origin[2];
     double  probe_step[2];

@@ -119,7 +119,7 @@ static int check_prism(const prism_params* p)
     const int mx = p->nx / p->f, my = p->ny / p->f;
     if (!is_pow2(mx) || !is_pow2(my)) return PRISM_EINVAL;
     if (mx < 16 || my < 16) return PRISM_EUNSUPPORTED;
-    if (mx * my > 128 * 128) return PRISM_EUNSUPPORTED;
+    if (mx > 128 || my > 128) return PRISM_EUNSUPPORTED;     // window_out holds 16 .. 128 points per side on chip
     return PRISM_OK;
 }
 

@@ -110,6 +110,11 @@ def test_argument_checks_without_a_gpu(prism):
     p = prism.params_from_workload(w, f=8)
     with pytest.raises(prism.PrismError):
         prism.workspace_bytes(p, prism.WS_OUTPUT)
+    # a window side above 128 points too, even when the window area is not (256 x 64 at 512 x 128, f = 2)
+    wide = prism.params_from_workload(w, nx=512, ny=128, f=2)
+    wide.cell[0], wide.cell[1] = 51.2, 12.8
+    assert prism.num_beams(wide) > 0
+    assert prism._lib.prism_workspace_bytes(C.byref(wide), prism.WS_OUTPUT) == 0
     assert prism._lib.prism_strerror(prism.PRISM_ENOMEM) == b"workspace too small"
 
 
