@@ -16,7 +16,8 @@
  * a function of its arguments.  What it does keep, process-wide, is bookkeeping:
  * per-device marks for one-time kernel set-up (shared-memory opt-in, occupancy), a
  * launch counter, and -- only while prism_timing_enable is on -- a list of timing
- * events.  Calls may be made concurrently from several host threads (one per device
+ * events (pooled per device: a launch takes its pair from the device current when it
+ * is enqueued).  Calls may be made concurrently from several host threads (one per device
  * or stream, the paper's multi-GPU model); the bookkeeping is atomic or
  * mutex-guarded.
  * Work is enqueued on the given stream; outputs are valid once the caller has
@@ -63,7 +64,11 @@ typedef struct prism_aberration {
 
 /* The paper's parameters (cell & pixel size PAPER.md:158,:182; slice thickness :158,:200; voltage :182;
  * probe semi-angle :200,:214; interpolation factor f :86; probe grid/step :174,:200; batch_size :126;
- * memory mode :138; annular detectors :82). */
+ * memory mode :138; annular detectors :82).
+ * The struct carries no size or version field: ZERO-INITIALISE it (memset / `= {0}`) and then set what you use, and
+ * rebuild callers against this header when it changes.  Fields added later (smatrix_on_host, n_aberrations,
+ * aberrations) mean "off" when zero; left uninitialised, n_aberrations / aberrations make the library read through
+ * a wild pointer (only the count's range, 0 .. 32, and a NULL pointer can be caught). */
 typedef struct prism_params {
     double  cell[3];            /* lx, ly, lz                                                              */
     int32_t nx, ny;             /* grid; pixel = cell / n; powers of two in [64, 2048]                      */
@@ -89,7 +94,9 @@ typedef struct prism_params {
                                    their layers out (copies overlapped with the next batch);
                                    prism_compute_output / _patterns / _detectors keep a ring of pixel rows in the
                                    workspace and bring in the rows the next batch of probe rows adds while the
-                                   current one computes.  Regular probe lattices only. */
+                                   current one computes (the copies overlap the kernels when consecutive
+                                   probe-row batches share or abut pixel rows, i.e. probe-row step <= window
+                                   side; otherwise they alternate with them).  Regular probe lattices only. */
     int32_t n_aberrations;      /* further terms of chi beside C1 and C3 (0 .. 32)                           */
     const prism_aberration* aberrations;   /* HOST array of n_aberrations terms (may be NULL when the count is 0) */
 } prism_params;
@@ -105,7 +112,11 @@ typedef struct prism_lut {
 } prism_lut;
 
 /* which = */
-enum { PRISM_WS_SMATRIX = 0, PRISM_WS_OUTPUT = 1, PRISM_WS_MULTISLICE = 2, PRISM_WS_POTENTIAL = 3 };
+enum { PRISM_WS_SMATRIX = 0, PRISM_WS_OUTPUT = 1, PRISM_WS_MULTISLICE = 2, PRISM_WS_POTENTIAL = 3,
+       PRISM_WS_MULTISLICE_PATTERNS = 4   /* multislice_compute_patterns / _detectors only: they never take the resident
+                                             route, so on 256^2 / 512^2 grids they need a batch of waves instead of one
+                                             wave per SM (PRISM_WS_MULTISLICE is enough for all three calls, and larger) */
+};
 
 /* Bytes of DEVICE workspace the corresponding call needs for these parameters (host-only, no CUDA). */
 size_t  prism_workspace_bytes(const prism_params* p, int32_t which);
@@ -191,7 +202,7 @@ int multislice_compute_output(const prism_params* p, const float* v, float* out,
  *   patterns OUT DEVICE fp32 [probes_y * probes_x][my][mx] (PRISM: mx = nx / f, my = ny / f, pattern pixel (ky, kx)
  *            at frequency (kx f / lx, ky f / ly); multislice: mx = nx, my = ny), array slot m = signed frequency
  *            index as for the DFT convention above; normalised like the ring output (a pattern sums to at most 1).
- *   Rings of prism_compute_output are sums of these pixels.  workspace: PRISM_WS_OUTPUT / PRISM_WS_MULTISLICE. */
+ *   Rings of prism_compute_output are sums of these pixels.  workspace: PRISM_WS_OUTPUT / PRISM_WS_MULTISLICE_PATTERNS. */
 int prism_compute_patterns(const prism_params* p, const void* s, const int32_t* beams, int32_t n_beams,
                            float* patterns, void* workspace, size_t workspace_bytes, void* cuda_stream);
 int multislice_compute_patterns(const prism_params* p, const float* v, float* patterns,
@@ -202,7 +213,7 @@ int multislice_compute_patterns(const prism_params* p, const float* v, float* pa
  * masks[d][ky][kx] * I[ky][kx], with the patterns of prism_compute_patterns / multislice_compute_patterns.
  *   masks IN  DEVICE fp32 [n_masks][my][mx] (weights; 0 / 1 for a plain detector), 1 <= n_masks <= 16
  *   out   OUT DEVICE fp32 [probes_y * probes_x][n_masks]
- * Fixed summation order (deterministic).  workspace: PRISM_WS_OUTPUT / PRISM_WS_MULTISLICE. */
+ * Fixed summation order (deterministic).  workspace: PRISM_WS_OUTPUT / PRISM_WS_MULTISLICE_PATTERNS. */
 int prism_compute_detectors(const prism_params* p, const void* s, const int32_t* beams, int32_t n_beams,
                             const float* masks, int32_t n_masks, float* out,
                             void* workspace, size_t workspace_bytes, void* cuda_stream);

@@ -39,37 +39,62 @@ enum KernelClass { K_POTENTIAL = 0, K_TRANSMISSION, K_ROW_INIT, K_ROW_STEP, K_RO
 static const char* const kClassNames[K_NUM_CLASSES] = {
     "potential", "transmission", "row_init", "row_step", "row_final", "col_step", "beam_sum",
     "bin_reduce", "col_ms_init", "col_ms_final", "lattice_dft", "patterns", "detectors", "accumulate", "window_out", "ms_resident" };
-struct TimedLaunch { int cls; cudaEvent_t e0, e1; };
-// The record is process-wide and guarded by a mutex that is taken only while timing is enabled.
+struct TimedLaunch { int cls, dev; cudaEvent_t e0, e1; };
+// The record is process-wide and guarded by a mutex that is taken only while timing is enabled.  Events belong to the
+// device they were created on: the pool of reusable events (creating them costs more than recording) is kept per
+// device, and a launch takes its pair from the pool of the device that is current when it is enqueued.
+constexpr int TIMING_MAX_DEVICES = 64;
 static std::atomic<bool> g_timing{false};
 static std::mutex g_timing_mu;
 static std::vector<TimedLaunch> g_timed;
-static std::vector<cudaEvent_t> g_event_pool;      // events are reused: creating them costs more than recording
-static cudaEvent_t take_event()
+static std::vector<cudaEvent_t> g_event_pool[TIMING_MAX_DEVICES];
+static cudaError_t take_event_pair(int* dev, cudaEvent_t* e0, cudaEvent_t* e1)
 {
+    cudaError_t e = cudaGetDevice(dev);
+    if (e != cudaSuccess) return e;
+    if (*dev < 0 || *dev >= TIMING_MAX_DEVICES) return cudaErrorInvalidDevice;
     std::lock_guard<std::mutex> lock(g_timing_mu);
-    cudaEvent_t e = nullptr;
-    if (!g_event_pool.empty()) { e = g_event_pool.back(); g_event_pool.pop_back(); }
-    else cudaEventCreate(&e);
-    return e;
+    std::vector<cudaEvent_t>& pool = g_event_pool[*dev];
+    cudaEvent_t* out[2] = {e0, e1};
+    for (int i = 0; i < 2; ++i) {
+        if (!pool.empty()) { *out[i] = pool.back(); pool.pop_back(); }
+        else if ((e = cudaEventCreate(out[i])) != cudaSuccess) {
+            if (i == 1) pool.push_back(*e0);
+            return e;
+        }
+    }
+    return cudaSuccess;
 }
-static void record_timed(int cls, cudaEvent_t e0, cudaEvent_t e1)
+static void return_event_pair(int dev, cudaEvent_t e0, cudaEvent_t e1)
 {
     std::lock_guard<std::mutex> lock(g_timing_mu);
-    g_timed.push_back({cls, e0, e1});
+    g_event_pool[dev].push_back(e0);
+    g_event_pool[dev].push_back(e1);
+}
+static void record_timed(int cls, int dev, cudaEvent_t e0, cudaEvent_t e1)
+{
+    std::lock_guard<std::mutex> lock(g_timing_mu);
+    g_timed.push_back({cls, dev, e0, e1});
 }
 
 #define LAUNCH(cls, call, stream)                                                      \
     do {                                                                               \
         cudaEvent_t e0__ = nullptr, e1__ = nullptr;                                    \
+        int dev__ = 0;                                                                 \
         const bool timed__ = g_timing.load(std::memory_order_relaxed);                 \
         if (timed__) {                                                                 \
-            e0__ = take_event(); e1__ = take_event();                                  \
-            cudaEventRecord(e0__, (stream));                                           \
+            cudaError_t t__ = take_event_pair(&dev__, &e0__, &e1__);                   \
+            if (t__ != cudaSuccess) return cuda_fail(t__, "timing events of " #call);  \
+            t__ = cudaEventRecord(e0__, (stream));                                     \
+            if (t__ != cudaSuccess) { return_event_pair(dev__, e0__, e1__); return cuda_fail(t__, "cudaEventRecord before " #call); } \
         }                                                                              \
         cudaError_t e__ = (call);                                                      \
-        if (e__ != cudaSuccess) return cuda_fail(e__, #call);                          \
-        if (timed__) { cudaEventRecord(e1__, (stream)); record_timed((cls), e0__, e1__); } \
+        if (e__ == cudaSuccess && timed__) e__ = cudaEventRecord(e1__, (stream));      \
+        if (e__ != cudaSuccess) {                                                      \
+            if (timed__) return_event_pair(dev__, e0__, e1__);                         \
+            return cuda_fail(e__, #call);                                              \
+        }                                                                              \
+        if (timed__) record_timed((cls), dev__, e0__, e1__);                           \
         g_launches.fetch_add(1, std::memory_order_relaxed);                            \
     } while (0)
 
@@ -567,7 +592,10 @@ static LatticePlan plan_lattice(const prism_params* p, const int32_t* beams, int
 // window row of probe row 0 (pixel row (y00 + u) mod ny); probe-row batch k needs u in [sy R k, sy R k + pix_k) and
 // row u sits at ring row u % cap.  Each batch copies only the rows the ring does not hold yet, on a private copy
 // stream: with cap >= rows of a batch + rows the next batch adds, the copies of batch k + 1 overlap the kernels of
-// batch k (they wait for batch k - 1, whose rows they overwrite).
+// batch k (they wait for batch k - 1, whose rows they overwrite).  That holds whenever consecutive batches share or
+// abut pixel rows (probe-row step <= window side, every lattice the configs use).  When they leave a gap
+// (sy * rows_per_batch > rows of a batch) the ring is 2 x a batch deep but row u % cap of batch k + 1 can land on rows
+// batch k still reads, so copy_batch(k + 1) waits for done[k]: correct, not overlapped.
 struct SlabRing {
     const char* s = nullptr;            // host S-matrix [n_beams][ny][nx] complex64
     char* slab = nullptr;               // device ring [n_beams][cap][nx]
@@ -646,14 +674,17 @@ static bool multislice_resident(const prism_params* p)
     return resident_grid(p->nx, p->ny) && !p->potential_on_host &&
            (size_t)p->n_slices * p->nx * p->ny * sizeof(float2) <= ((size_t)256 << 20);
 }
-static void layout_multislice(Arena& a, const prism_params* p, MultisliceLayout& L)
+// `rings`: the call integrates into rings and so may take the resident route; patterns and mask detectors always
+// run per pass and need a batch of waves only.  RESIDENT_SLOTS is a cap on the waves in flight (the launch takes
+// min(probes, slots, SMs of the device)), kept a constant so that prism_workspace_bytes stays host-only.
+static void layout_multislice(Arena& a, const prism_params* p, MultisliceLayout& L, bool rings)
 {
     const size_t npix = (size_t)p->nx * p->ny;
     const int nb = prism_num_bins(p);
     L.batch = default_probe_batch(p, npix * 12);
     // wave slots: a batch of the per-pass path, or one per SM for the resident kernel
     L.waves = L.batch;
-    if (multislice_resident(p))
+    if (rings && multislice_resident(p))
         L.waves = std::max<long long>(L.batch, std::min<long long>((long long)p->probes_x * p->probes_y, RESIDENT_SLOTS));
     carve_slice_tables(a, p, L.tab);
     carve_feeder(a, p, L.feed, true);
@@ -769,16 +800,20 @@ int prism_timing_read(double* ms_by_class, int64_t* launches_by_class)
     if (!ms_by_class || !launches_by_class) return PRISM_EINVAL;
     for (int c = 0; c < K_NUM_CLASSES; ++c) { ms_by_class[c] = 0.0; launches_by_class[c] = 0; }
     std::lock_guard<std::mutex> lock(g_timing_mu);
-    for (const TimedLaunch& t : g_timed) {
-        CU(cudaEventSynchronize(t.e1));
+    // every entry leaves the record as it is read and its events go back to their device's pool exactly once, also
+    // when a CUDA call fails part-way: the entries not yet read stay for the next call
+    while (!g_timed.empty()) {
+        const TimedLaunch t = g_timed.back();
+        g_timed.pop_back();
         float ms = 0.f;
-        CU(cudaEventElapsedTime(&ms, t.e0, t.e1));
+        cudaError_t e = cudaEventSynchronize(t.e1);
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, t.e0, t.e1);
+        g_event_pool[t.dev].push_back(t.e0);
+        g_event_pool[t.dev].push_back(t.e1);
+        if (e != cudaSuccess) return cuda_fail(e, "prism_timing_read");
         ms_by_class[t.cls] += ms;
         ++launches_by_class[t.cls];
-        g_event_pool.push_back(t.e0);
-        g_event_pool.push_back(t.e1);
     }
-    g_timed.clear();
     return PRISM_OK;
 }
 
@@ -845,7 +880,13 @@ size_t prism_workspace_bytes(const prism_params* p, int32_t which)
         case PRISM_WS_MULTISLICE: {
             if (check_probe(p)) return 0;
             MultisliceLayout L;
-            layout_multislice(a, p, L);
+            layout_multislice(a, p, L, true);
+            break;
+        }
+        case PRISM_WS_MULTISLICE_PATTERNS: {
+            if (check_probe(p)) return 0;
+            MultisliceLayout L;
+            layout_multislice(a, p, L, false);
             break;
         }
         case PRISM_WS_POTENTIAL: {
@@ -1310,7 +1351,7 @@ static int multislice_impl(const prism_params* p, const float* v, float* out, fl
 
     Arena a(workspace, workspace_bytes);
     MultisliceLayout L;
-    layout_multislice(a, p, L);
+    layout_multislice(a, p, L, out != nullptr);
     if (!a.ok()) return PRISM_ENOMEM;
     const bool out_dev = out ? pointer_is_device(out) : true;
     float* d_out = out_dev ? out : L.out_stage;

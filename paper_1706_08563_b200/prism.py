@@ -17,7 +17,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.environ.get("PRISM_B200_LIB") or os.path.join(_HERE, "libprism_b200.so")
 
 PRISM_OK, PRISM_EINVAL, PRISM_ENOMEM, PRISM_ECUDA, PRISM_EUNSUPPORTED, PRISM_ENOLUT = 0, -1, -2, -3, -4, -5
-WS_SMATRIX, WS_OUTPUT, WS_MULTISLICE, WS_POTENTIAL = 0, 1, 2, 3
+WS_SMATRIX, WS_OUTPUT, WS_MULTISLICE, WS_POTENTIAL, WS_MULTISLICE_PATTERNS = 0, 1, 2, 3, 4
 
 EXPORTS = ["prism_workspace_bytes", "prism_num_bins", "prism_num_beams", "prism_band_columns", "prism_constants",
            "prism_build_potential", "prism_build_potential_static", "prism_compute_smatrix", "prism_compute_output",

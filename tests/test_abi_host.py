@@ -86,8 +86,15 @@ def test_band_columns_cover_the_oracle_propagator(prism, name):
 def test_workspace_sizes_are_positive_and_scale(prism):
     w = W.get("P4")
     p = prism.params_from_workload(w)
-    sizes = [prism.workspace_bytes(p, k) for k in range(4)]
+    sizes = [prism.workspace_bytes(p, k) for k in range(5)]
     assert all(s > 0 for s in sizes)
+    # 512^2 is a resident-multislice grid: ring output keeps a wave per SM, patterns / detectors a batch only
+    assert sizes[prism.WS_MULTISLICE_PATTERNS] <= sizes[prism.WS_MULTISLICE]
+    few = prism.params_from_workload(w, batch=4)
+    assert (prism.workspace_bytes(few, prism.WS_MULTISLICE) - prism.workspace_bytes(few, prism.WS_MULTISLICE_PATTERNS)
+            == (148 - 4) * 512 * 512 * 12)
+    small = prism.params_from_workload(W.pr1())                     # 64^2 never runs resident: the two agree
+    assert prism.workspace_bytes(small, prism.WS_MULTISLICE_PATTERNS) == prism.workspace_bytes(small, prism.WS_MULTISLICE)
     assert sizes[prism.WS_SMATRIX] < 64 << 20                       # tables + one t slice only
     p_host = prism.params_from_workload(w, potential_on_host=1)
     assert prism.workspace_bytes(p_host, prism.WS_SMATRIX) == sizes[0] + 3 * 512 * 512 * 4

@@ -48,7 +48,7 @@ def _ms_patterns(G, w, v, p=None):
     from paper_1706_08563_b200 import prism
     p = p or prism.params_from_workload(w)
     pat = torch.empty((w.n_probes, w.ny, w.nx), dtype=torch.float32, device=G.DEV)
-    prism.multislice_patterns(p, v, pat, G.ws(p, prism.WS_MULTISLICE))
+    prism.multislice_patterns(p, v, pat, G.ws(p, prism.WS_MULTISLICE_PATTERNS))
     torch.cuda.synchronize()
     return pat.cpu().numpy().astype(np.float64)
 
@@ -172,7 +172,7 @@ def test_multislice_detectors_parity(G):
     masks = _masks(w, p, w.ny, w.nx, 1, 1, np.random.default_rng(6))
     m_dev = torch.as_tensor(masks, dtype=torch.float32, device=G.DEV).contiguous()
     out = torch.empty((w.n_probes, len(masks)), dtype=torch.float32, device=G.DEV)
-    prism.multislice_detectors(pp, v, m_dev, out, G.ws(pp, prism.WS_MULTISLICE))
+    prism.multislice_detectors(pp, v, m_dev, out, G.ws(pp, prism.WS_MULTISLICE_PATTERNS))
     torch.cuda.synchronize()
     got = out.cpu().numpy().astype(np.float64)
     v_ref = oracle_potential(w)

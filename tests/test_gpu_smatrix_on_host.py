@@ -1,6 +1,7 @@
 """S-matrix in page-locked host memory (PAPER.md:136 streaming PRISM: the device holds only
 "the current S-matrix subset").  Stage 1 propagates `batch` beams at a time in the workspace and copies their layers
-out; stage 2 copies, per batch of probe rows, the pixel rows of every layer that those rows' windows cover.  Both must
+out from alternating buffers; stage 2 keeps a ring of pixel rows of every layer in the workspace and brings in, on a
+private copy stream, only the rows the next batch of probe rows adds while the current batch computes.  Both must
 reproduce the resident path bit for bit, and through it the oracle."""
 import numpy as np
 import pytest
