@@ -22,7 +22,7 @@ __all__ = [
     "Params", "build", "constants", "dft_naive", "fft", "fft2", "dft2_naive",
     "potential", "transmission", "propagator", "slice_step", "multislice_wave",
     "num_aperture", "probe", "num_bins", "bin_intensity", "multislice_probe",
-    "beams", "smatrix_layer", "smatrix", "prism_probe", "multislice_probes",
+    "beams", "smatrix_layer", "smatrix", "prism_probe", "prism_probe_rows", "multislice_probes",
     "prism_probes", "num_threads",
 ]
 
@@ -268,6 +268,24 @@ def prism_probe(p: Params, s, beam_list, xp: float, yp: float, use_naive: bool =
     _L().orc_prism_probe(C.byref(cp), _p(s), _p(beam_list), C.c_int(len(beam_list)),
                          C.c_double(xp), C.c_double(yp), _p(out),
                          _p(pat) if want_pattern else None, C.c_int(int(use_naive)))
+    return (out, pat) if want_pattern else out
+
+
+def prism_probe_rows(p: Params, s_rows, row0: int, beam_list, xp: float, yp: float,
+                     want_pattern: bool = False):
+    """``prism_probe`` when only pixel rows ``[row0, row0 + n_rows)`` (mod ny) of every layer are in memory:
+    ``s_rows[b][r]`` = pixel row ``(row0 + r) % ny`` of layer b (storage only; same loop and arithmetic)."""
+    s_rows = _c128(s_rows)
+    beam_list = np.ascontiguousarray(beam_list, dtype=np.int32).reshape(-1, 2)
+    assert s_rows.ndim == 3 and s_rows.shape[0] == len(beam_list) and s_rows.shape[2] == p.nx
+    out = np.empty(num_bins(p), dtype=np.float64)
+    pat = np.empty((p.ny // p.f, p.nx // p.f), dtype=np.float64) if want_pattern else None
+    cp = p.c()
+    rc = _L().orc_prism_probe_rows(C.byref(cp), _p(s_rows), C.c_int(int(row0)), C.c_int(s_rows.shape[1]),
+                                   _p(beam_list), C.c_int(len(beam_list)), C.c_double(xp), C.c_double(yp),
+                                   _p(out), _p(pat) if want_pattern else None, C.c_int(0))
+    if rc != 0:
+        raise ValueError("the probe's window leaves the band of rows")
     return (out, pat) if want_pattern else out
 
 

@@ -415,12 +415,29 @@ void orc_prism_probe(const orc_params *p, const orc_c128 *s, const int32_t *beam
                      int n_beams, double xp, double yp, double *out_bins,
                      double *pattern, int use_naive)
 {
+    /* the whole grid is the band of rows [0, ny) */
+    orc_prism_probe_rows(p, s, 0, p->ny, beams, n_beams, xp, yp, out_bins, pattern, use_naive);
+}
+
+/* The same probe when only a band of pixel rows of every layer is in memory
+ * (storage only, no new reading: at 2048^2 x 1201 beams the whole fp64
+ * S-matrix is 80 GB, the 128 rows one probe's window touches are 5 GB).
+ * s_rows[b][r][i] holds pixel row (row0 + r) mod ny of layer b, r < n_rows.
+ * Returns 0, or -1 (nothing written) if the probe's window leaves the band. */
+int orc_prism_probe_rows(const orc_params *p, const orc_c128 *s_rows, int row0, int n_rows,
+                         const int32_t *beams, int n_beams, double xp, double yp,
+                         double *out_bins, double *pattern, int use_naive)
+{
     double lambda; orc_constants(p->voltage, &lambda, NULL);
     const int nx = p->nx, ny = p->ny, f = p->f;
     const int mx_n = nx / f, my_n = ny / f;
-    size_t n = (size_t)nx * ny, m = (size_t)mx_n * my_n;
+    size_t n = (size_t)nx * n_rows, m = (size_t)mx_n * my_n;
     const double px = p->lx / nx, py = p->ly / ny;
     int ic = (int)floor(xp / px + 0.5), jc = (int)floor(yp / py + 0.5);
+    for (int j = 0; j < my_n; ++j) {
+        int jw = (((jc - my_n / 2 + j) % ny) + ny) % ny;
+        if ((((jw - row0) % ny) + ny) % ny >= n_rows) return -1;
+    }
     orc_c128 *w = (orc_c128 *)calloc(m, sizeof(orc_c128));
     double *inten = (double *)malloc(sizeof(double) * m);
     for (int b = 0; b < n_beams; ++b) {
@@ -428,13 +445,14 @@ void orc_prism_probe(const orc_params *p, const orc_c128 *s, const int32_t *beam
         double qx = kx / p->lx, qy = ky / p->ly;
         double phase = -chi(p, lambda, qx, qy) - 2.0 * ORC_PI * (qx * xp + qy * yp);
         orc_c128 coef = c_expi(phase);
-        const orc_c128 *layer = s + (size_t)b * n;
+        const orc_c128 *layer = s_rows + (size_t)b * n;
         for (int j = 0; j < my_n; ++j) {
             int jw = (((jc - my_n / 2 + j) % ny) + ny) % ny;
+            int jr = (((jw - row0) % ny) + ny) % ny;       /* where pixel row jw sits in the band */
             for (int i = 0; i < mx_n; ++i) {
                 int iw = (((ic - mx_n / 2 + i) % nx) + nx) % nx;
                 w[(size_t)j * mx_n + i] = c_add(w[(size_t)j * mx_n + i],
-                                                c_mul(coef, layer[(size_t)jw * nx + iw]));
+                                                c_mul(coef, layer[(size_t)jr * nx + iw]));
             }
         }
     }
@@ -445,6 +463,7 @@ void orc_prism_probe(const orc_params *p, const orc_c128 *s, const int32_t *beam
     orc_bin_intensity(p, inten, my_n, mx_n, f, f, out_bins);
     if (pattern) memcpy(pattern, inten, sizeof(double) * m);
     free(w); free(inten);
+    return 0;
 }
 
 /* ------------------------------------------------------------------------- */

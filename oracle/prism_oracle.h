@@ -102,6 +102,11 @@ void   orc_smatrix(const orc_params *p, const double *v, const int32_t *beams, i
 void   orc_prism_probe(const orc_params *p, const orc_c128 *s, const int32_t *beams,
                        int n_beams, double xp, double yp, double *out_bins,
                        double *pattern, int use_naive);
+/* the same with only pixel rows [row0, row0 + n_rows) (mod ny) of every layer in memory:
+ * s_rows[b][r][i] = layer b, pixel row (row0 + r) mod ny.  -1 if the window leaves the band. */
+int    orc_prism_probe_rows(const orc_params *p, const orc_c128 *s_rows, int row0, int n_rows,
+                            const int32_t *beams, int n_beams, double xp, double yp,
+                            double *out_bins, double *pattern, int use_naive);
 
 /* batched drivers (OpenMP over probes); out[probe][bin] */
 void   orc_multislice_probes(const orc_params *p, const double *v, const double *xy,

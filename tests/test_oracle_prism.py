@@ -292,3 +292,66 @@ def test_batched_drivers_equal_single_calls():
         assert np.array_equal(ms[i], O.multislice_probe(p, v, xp, yp))
         assert np.array_equal(pr[i], O.prism_probe(p, s, b, xp, yp))
     assert np.array_equal(s[3], O.smatrix_layer(p, v, *b[3]))
+
+
+# ----------------------------------------------------------------------------- band-of-rows storage (O10, storage only)
+def _band(s, row0, n_rows):
+    ny = s.shape[1]
+    return np.ascontiguousarray(s[:, (row0 + np.arange(n_rows)) % ny, :])
+
+
+@pytest.mark.parametrize("f", [1, 4])
+def test_prism_probe_rows_is_bit_identical_to_the_whole_grid(f):
+    """orc_prism_probe_rows sees only the pixel rows [row0, row0 + n_rows) of every layer; for any band that holds the
+    probe's window it must give the whole-grid result bit for bit (same loop, same order): PR1 (f = 1: the band is the
+    whole grid, rotated), an f = 4 window inside a band, and a band that wraps the cell edge."""
+    w = W.pr1()
+    p = oracle_params(w) if f == 1 else params(64, f=4, alpha=30e-3)
+    rng = np.random.default_rng(99)
+    b = O.beams(p)
+    if f == 1:
+        s = O.smatrix(p, oracle_potential(w), b)
+    else:
+        s = rng.normal(size=(len(b), 64, 64)) + 1j * rng.normal(size=(len(b), 64, 64))
+    m = 64 // f
+    for xp, yp in [(2.0, 3.0), (0.0, 0.0), (6.35, 0.25), (1.23, 5.9)]:
+        want, want_pat = O.prism_probe(p, s, b, xp, yp, want_pattern=True)
+        jc = int(np.floor(yp / 0.1 + 0.5))
+        first = (jc - m // 2) % 64                         # first pixel row of the window (R8)
+        bands = [(first, m), ((first - 3) % 64, min(64, m + 7))] if f > 1 else [(first, 64), (17, 64)]
+        for row0, n_rows in bands:
+            got, got_pat = O.prism_probe_rows(p, _band(s, row0, n_rows), row0, b, xp, yp, want_pattern=True)
+            assert np.array_equal(got, want) and np.array_equal(got_pat, want_pat), (xp, yp, row0, n_rows)
+    # the probe at the origin with f = 4: window rows [-8, 8) -> band starts at pixel row 56 and wraps through 0
+    if f == 4:
+        got = O.prism_probe_rows(p, _band(s, 56, 16), 56, b, 0.0, 0.0)
+        assert np.array_equal(got, O.prism_probe(p, s, b, 0.0, 0.0))
+        # a band that misses one window row is refused, not read out of bounds
+        with pytest.raises(ValueError):
+            O.prism_probe_rows(p, _band(s, 57, 16), 57, b, 0.0, 0.0)
+        with pytest.raises(ValueError):
+            O.prism_probe_rows(p, _band(s, 56, 15), 56, b, 0.0, 0.0)
+
+
+def test_prism_probe_rows_placement_with_a_point_band():
+    """Independent of the whole-grid routine: a single non-zero pixel at band row r stands for pixel row
+    (row0 + r) mod ny; it contributes iff that pixel row lies in the probe's window, with the Parseval weight."""
+    n, f = 64, 4
+    m = n // f
+    p = params(n, f=f, alpha=30e-3)
+    b = O.beams(p)
+    nb = len(b)
+    xp, yp = 2.0, 0.3                                     # centre pixel (20, 3) -> window rows [-5, 11)
+    row0, n_rows = 50, 30                                 # band = pixel rows 50 .. 63, 0 .. 15
+    coef = np.exp(-2j * np.pi * (b[:, 0] * xp + b[:, 1] * yp) / 6.4)
+    inside = abs(coef.sum()) ** 2 / (nb * m * m)
+
+    def total(r, i0):
+        s = np.zeros((nb, n_rows, n), complex)
+        s[:, r, i0] = 1.0
+        return O.prism_probe_rows(p, s, row0, b, xp, yp, want_pattern=True)[1].sum()
+
+    assert abs(total(9, 20) - inside) < 1e-12             # pixel row 59 = -5: first row of the window
+    assert abs(total(24, 27) - inside) < 1e-12            # pixel row 10: last row, last column [12, 28)
+    assert total(8, 20) == 0.0 and total(25, 20) == 0.0   # pixel rows 58 and 11: just outside
+    assert total(14, 28) == 0.0 and total(14, 11) == 0.0  # inside in y (pixel row 0), outside in x
