@@ -200,6 +200,18 @@ def p16_multislice() -> Workload:
     return w.with_(name="P16-MS", probes_x=64, probes_y=64, probe_step=(3.2, 3.2))
 
 
+def p16_first_slices(n_slices: int) -> Workload:
+    """Config 5 cut to its first `n_slices` slices (for oracle runs that cannot afford all 400): atoms above the
+    truncated stack are dropped (not clamped into the last slice), the cell height follows; grid, beams, probe
+    lattice and the streamed potential are config 5's."""
+    w = p16()
+    if n_slices >= w.n_slices:
+        return w
+    keep = w.atoms[:, 2] < n_slices * w.dz - 1.0
+    return w.with_(n_slices=n_slices, atoms=w.atoms[keep], z=w.z[keep],
+                   cell=(w.cell[0], w.cell[1], n_slices * w.dz))
+
+
 CONFIGS = {"PR1": pr1, "MS2": ms2, "P4": p4, "P8": p8, "P16": p16, "P16-MS": p16_multislice}
 
 

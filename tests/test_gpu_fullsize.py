@@ -86,7 +86,38 @@ def check_prism(G, w, n_layers, n_probes, beam_filter=None, tol_out=TOL_OUT):
     # norm-conserving for f > 1, so this is a sanity band, not an identity)
     tot = out.sum(axis=1)
     assert np.all(tot > 0.5) and np.all(tot < 1.05)
+    if beam_filter is not None:
+        check_stage2_all_beams_on_row_bands(G, w, p, s, beams, tol_out)
     return v, v_ref, errs
+
+
+def check_stage2_all_beams_on_row_bands(G, w, p, s, beams, tol_out, n_probes=8):
+    """Stage 2 with EVERY beam at sizes where the fp64 copy of the whole S-matrix does not fit in host memory (80 GB at
+    config 5): for one probe row, only the ny / f pixel rows its windows touch are brought to the host in fp64 (5 GB at
+    config 5) and the oracle's band-of-rows entry (O.prism_probe_rows: the loop of O.prism_probe on that storage) gives
+    the rings of sampled probes of the row.  Two probe rows: probe row 0, whose windows wrap the cell edge in y, and one
+    in the middle of the grid."""
+    out = G.gpu_prism_output(w, s, beams)                  # all beams, the launch configuration bench.py times
+    xy = w.probe_xy().reshape(w.probes_y, w.probes_x, 2)
+    my, py = w.ny // w.f, w.cell[1] / w.ny
+    d = G.dark_field(w, p)
+    for iy in (0, (w.probes_y // 2) + 3):
+        jc = int(np.floor(xy[iy, 0, 1] / py + 0.5))
+        row0 = (jc - my // 2) % w.ny
+        if iy == 0:
+            assert row0 + my > w.ny                        # this band wraps the cell edge
+        idx = torch.as_tensor((row0 + np.arange(my)) % w.ny, device=s.device)
+        band = s.index_select(1, idx).cpu().numpy().astype(np.complex128)
+        cols = spread(w.probes_x, n_probes)
+        ref = np.stack([O.prism_probe_rows(p, band, row0, beams, *xy[iy, ix]) for ix in cols])
+        del band
+        got = out.reshape(w.probes_y, w.probes_x, -1)[iy, cols]
+        e, e_dark = rel_l2(got, ref), rel_l2(got[:, d:], ref[:, d:])
+        print(f"{w.name} stage 2, all {len(beams)} beams, probe row {iy} (band from pixel row {row0}): "
+              f"rings {e:.3e}, dark field {e_dark:.3e}")
+        assert e < TOL_STAGE2, iy
+        assert ref[:, d:].sum() > 0
+        assert e_dark < 5 * tol_out, iy
 
 
 def check_multislice(G, w, v, v_ref, n_probes, tol_out=TOL_OUT):
@@ -151,11 +182,7 @@ def test_p8_full(G):
 def p16_cases(n_slices):
     """Config 5 on its first n_slices slices: atoms above the truncated stack are dropped (not clamped into the
     last slice), everything else -- grid, beams, streamed potential, probe lattices -- is config 5."""
-    w = W.p16()
-    if n_slices < w.n_slices:
-        keep = w.atoms[:, 2] < n_slices * w.dz - 1.0
-        w = w.with_(n_slices=n_slices, atoms=w.atoms[keep], z=w.z[keep],
-                    cell=(w.cell[0], w.cell[1], n_slices * w.dz))
+    w = W.p16_first_slices(n_slices)
     wm = w.with_(name="P16-MS", probes_x=64, probes_y=64, probe_step=(3.2, 3.2))
     return w, wm
 
@@ -179,16 +206,21 @@ def test_p16_first_40_slices(G):
 
 
 class _P16OracleJob:
-    """The two 400-slice oracle waves of config 5 (one S-matrix layer, one multislice probe; 4-9 min each on one core),
-    started on host threads when the module's first test begins, so that they overlap the other full-size tests."""
+    """The 400-slice oracle waves of config 5: three S-matrix layers (the axial beam, an oblique one, one on the
+    aperture edge) and two multislice probes, 4-9 min each on one core, each on its own host thread from the moment
+    the module's first test begins, so that they overlap the other full-size tests."""
 
     def __init__(self):
         self.w, self.wm = p16_cases(400)
         self.p, self.pm = oracle_params(self.w), oracle_params(self.wm)
         self.beams_ref = O.beams(self.p)
-        self.b_pick = len(self.beams_ref) // 3             # an oblique beam (not the central one)
+        b = self.beams_ref.astype(np.int64)
+        q2 = b[:, 0] ** 2 + b[:, 1] ** 2
+        self.b_picks = {"axial": int(np.argmin(q2)), "oblique": len(b) // 3, "edge": int(np.argmax(q2))}
+        assert q2[self.b_picks["axial"]] == 0 and len(set(self.b_picks.values())) == 3
         self.xy = self.wm.probe_xy()
-        self.i_probe = int(spread(len(self.xy), 5)[2]) + 7  # away from the cell corner and from lattice symmetry points
+        i_mid = int(spread(len(self.xy), 5)[2]) + 7        # away from the cell corner and from lattice symmetry points
+        self.i_probes = [i_mid, int(spread(len(self.xy), 5)[1]) + 29]
         self.ref, self.v_ref, self.error = {}, None, None
         self.thread = threading.Thread(target=self._run, daemon=True)
         self.thread.start()
@@ -197,14 +229,15 @@ class _P16OracleJob:
         try:
             self.v_ref = oracle_potential(self.w)          # ctypes releases the GIL inside the oracle calls
 
-            def layer():
-                kx, ky = (int(x) for x in self.beams_ref[self.b_pick])
-                self.ref["layer"] = O.smatrix_layer(self.p, self.v_ref, kx, ky)
+            def layer(name):
+                kx, ky = (int(x) for x in self.beams_ref[self.b_picks[name]])
+                self.ref["layer_" + name] = O.smatrix_layer(self.p, self.v_ref, kx, ky)
 
-            def probe():
-                self.ref["rings"] = O.multislice_probes(self.pm, self.v_ref, self.xy[self.i_probe:self.i_probe + 1])[0]
+            def probe(i):
+                self.ref["rings_%d" % i] = O.multislice_probe(self.pm, self.v_ref, *self.xy[i])
 
-            ts = [threading.Thread(target=layer), threading.Thread(target=probe)]
+            ts = [threading.Thread(target=layer, args=(name,)) for name in self.b_picks]
+            ts += [threading.Thread(target=probe, args=(i,)) for i in self.i_probes]
             for t in ts:
                 t.start()
             for t in ts:
@@ -283,19 +316,22 @@ def test_p8_end_to_end_full_oracle(G):
 
 def test_p16_full_400_slices(G, p16_oracle_job):
     """Config 5 at its full depth (2048^2, all 400 slices streamed from pinned host memory, 1201 beams resident):
-    one S-matrix layer against the oracle's, and one probe of the 64 x 64 multislice run end to end against the
-    oracle's rings at the 1e-3 of BASELINE.json north_star ("1e-3 for 2048^2 grids with >= 400 slices").  The two
-    oracle waves (400 slices each, ~4-9 min on one core) run on host threads from the start of this module."""
+    three S-matrix layers (axial, oblique, aperture-edge beam) against the oracle's, and two probes of the 64 x 64
+    multislice run end to end against the oracle's rings at the 1e-3 of BASELINE.json north_star ("1e-3 for 2048^2
+    grids with >= 400 slices").  The five oracle waves (400 slices each, ~4-9 min on one core) run on host threads
+    from the start of this module."""
     job = p16_oracle_job
     w, wm, p, pm = job.w, job.wm, job.p, job.pm
     assert w.n_slices == 400 and w.potential_on_host == 1
-    beams_ref, b_pick, i_probe = job.beams_ref, job.b_pick, job.i_probe
+    beams_ref = job.beams_ref
     try:
         v = G.gpu_potential(w, on_host=True)
         s, beams = G.gpu_smatrix(w, v)
         assert np.array_equal(beams, beams_ref) or set(map(tuple, beams.tolist())) == set(map(tuple, beams_ref.tolist()))
-        b_gpu = int(np.nonzero((beams == beams_ref[b_pick]).all(axis=1))[0][0])
-        layer_gpu = s[b_gpu].cpu().numpy().astype(np.complex128)
+        layers_gpu = {}
+        for name, b_pick in job.b_picks.items():
+            b_gpu = int(np.nonzero((beams == beams_ref[b_pick]).all(axis=1))[0][0])
+            layers_gpu[name] = s[b_gpu].cpu().numpy().astype(np.complex128)
         del s
         torch.cuda.empty_cache()
         out = G.gpu_multislice(wm, v)
@@ -304,13 +340,13 @@ def test_p16_full_400_slices(G, p16_oracle_job):
     assert job.error is None, job.error
     ref = job.ref
     assert rel_l2(v.numpy().astype(np.float64), job.v_ref) < TOL_V
-    e_layer = rel_l2(layer_gpu, ref["layer"])
-    e_rings = rel_l2(out[i_probe], ref["rings"])
+    e_layers = {name: rel_l2(layers_gpu[name], ref["layer_" + name]) for name in job.b_picks}
     d = G.dark_field(wm, pm)
-    e_dark = rel_l2(out[i_probe][d:], ref["rings"][d:])
-    print(f"P16 x 400 slices: S-matrix layer {e_layer:.3e}, multislice rings {e_rings:.3e}, dark field {e_dark:.3e}")
-    assert e_layer < tol_layer(400), e_layer
-    assert e_rings < 1e-3 and e_dark < 5e-3, (e_rings, e_dark)
+    e_rings = [rel_l2(out[i], ref["rings_%d" % i]) for i in job.i_probes]
+    e_dark = [rel_l2(out[i][d:], ref["rings_%d" % i][d:]) for i in job.i_probes]
+    print(f"P16 x 400 slices: S-matrix layers {e_layers}, multislice rings {e_rings}, dark field {e_dark}")
+    assert max(e_layers.values()) < tol_layer(400), e_layers
+    assert max(e_rings) < 1e-3 and max(e_dark) < 5e-3, (e_rings, e_dark)
     tot = out.sum(axis=1)
     assert np.all(tot > 0.0) and np.all(tot < 1.0 + 1e-3)
     job.v_ref = None
