@@ -33,20 +33,18 @@ def _deps_mtime() -> float:
     return max(os.path.getmtime(f) for f in files)
 
 
-def build(force: bool = False, verbose: bool = False, extra_flags=(), lib_path: str | None = None) -> str:
-    """Compile every .cu for sm_100a and link the C-ABI shared library.  `extra_flags` (e.g. ``-DNAME=value``
-    switches of csrc/) and `lib_path` build a variant beside the product library, for kernel experiments."""
-    variant = bool(extra_flags) or lib_path is not None
-    lib = lib_path or LIB
-    if not force and not variant and os.path.exists(lib) and os.path.getmtime(lib) >= _deps_mtime():
+def build(force: bool = False, verbose: bool = False) -> str:
+    """Compile every .cu for sm_100a and link the C-ABI shared library."""
+    lib = LIB
+    if not force and os.path.exists(lib) and os.path.getmtime(lib) >= _deps_mtime():
         return lib
-    obj_dir = OBJ if not variant else os.path.join(OBJ, "variant_" + os.path.basename(lib).replace(".", "_"))
+    obj_dir = OBJ
     os.makedirs(obj_dir, exist_ok=True)
     nvcc = _nvcc()
 
     def compile_one(src: str) -> str:
         obj = os.path.join(obj_dir, src.replace(".cu", ".o"))
-        cmd = [nvcc, *NVCC_FLAGS, *extra_flags, "-c", os.path.join(CSRC, src), "-o", obj]
+        cmd = [nvcc, *NVCC_FLAGS, "-c", os.path.join(CSRC, src), "-o", obj]
         if verbose:
             cmd.insert(1, "-Xptxas=-v")
         subprocess.check_call(cmd)

@@ -22,9 +22,7 @@
 
 namespace prism {
 
-#ifndef COL_TILE_PTS
-#define COL_TILE_PTS 8192
-#endif
+constexpr int COL_TILE_PTS = 8192;
 
 // =============================================================================
 // Column pass

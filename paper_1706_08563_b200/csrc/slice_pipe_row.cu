@@ -27,9 +27,7 @@
 
 namespace prism {
 
-#ifndef ROW_MAX_TEAMS
-#define ROW_MAX_TEAMS 16
-#endif
+constexpr int ROW_MAX_TEAMS = 16;
 
 // =============================================================================
 // Row pass

@@ -37,9 +37,7 @@ namespace prism {
 
 using pk::C2;
 
-#ifndef PK_ROW_MAX_WARPS
-#define PK_ROW_MAX_WARPS 8
-#endif
+constexpr int PK_ROW_MAX_WARPS = 8;
 
 // =============================================================================
 // Row pass
@@ -251,12 +249,8 @@ cudaError_t launch_row_pk(RowMode mode, const RowArgs& g, cudaStream_t stream)
 // i.e. runs of G x 64 B per tile.  Every warp of a CTA then needs the same row of the transmission function for
 // n_waves / 8 lines in a row: it is brought into shared memory once per row block (one bulk copy), which takes the
 // t_s loads out of the L1 / long-scoreboard path.
-// LOADER: the line is gathered by one 4-D TMA tensor box {8 columns, 1 row, 2 xb / 8 tiles, 1 wave} issued by one
-// lane (LAY_B8_TMA), or by 16-byte cp.async copies of all lanes (LAY_B8_CPA).
-#ifndef PRISM_B8_ROW_UNROLL_PH
-#define PRISM_B8_ROW_UNROLL_PH 0
-#endif
-enum { LAY_B8_CPA = 1, LAY_B8_TMA = 2 };
+// The line is gathered by one 4-D TMA tensor box {8 columns, 1 row, 2 xb / 8 tiles, 1 wave} issued by one lane
+// (16-byte cp.async copies by all lanes were measured slower: DESIGN.md 7.8).
 __device__ __forceinline__ void tensor_g2s_4d(void* smem_dst, const CUtensorMap* map, int c0, int c1, int c2, int c3,
                                               uint64_t* bar)
 {
@@ -277,7 +271,7 @@ struct RowB8Cfg {
     static constexpr size_t SMEM = PIPE_HEADER + TWB + T_BYTES + (size_t)WARPS * PER_WARP;
 };
 
-template <int N, int MODE, int XBE, int LOADER>
+template <int N, int MODE, int XBE>
 __global__ void __launch_bounds__(RowB8Cfg<N, XBE>::THREADS, 1) row_b8_kernel(RowArgs g, const __grid_constant__ CUtensorMap tmap)
 {
     using C = RowB8Cfg<N, XBE>;
@@ -296,7 +290,7 @@ __global__ void __launch_bounds__(RowB8Cfg<N, XBE>::THREADS, 1) row_b8_kernel(Ro
 
     pk::fill_tables<P>(tab, g.tw_x, tid, C::THREADS);
     if (lane == 0) {
-        if (MODE != ROW_INIT) mbar_init(&bars[warp], LOADER == LAY_B8_CPA ? 32 : 1);
+        if (MODE != ROW_INIT) mbar_init(&bars[warp], 1);
         if (warp == 0) mbar_init(tbar, 1);
         mbar_fence_init();
     }
@@ -314,32 +308,18 @@ __global__ void __launch_bounds__(RowB8Cfg<N, XBE>::THREADS, 1) row_b8_kernel(Ro
     const long long my_lines = (long long)my_yblocks * my_wgroups;
 
     // start the copies of line group `seq` into the landing buffer (compact: [0, xb) then [N - xb, N)).
-    // LAY_B8_CPA: called by every lane of the warp; LAY_B8_TMA: by lane 0.
+    // Called by lane 0.
     auto issue = [&](long long seq) {
         const int y = (int)(seq / my_wgroups) * G + bid, w0 = ((int)(seq % my_wgroups) * WARPS + warp) * LPW;
-        if (LOADER == LAY_B8_CPA) {
+        int n_act = 0;
 #pragma unroll
-            for (int l = 0; l < LPW; ++l) {
-                if (w0 + l < g.n_waves) {
-                    const float2* src = g.a + (size_t)(w0 + l) * wave_stride + (size_t)y * 8;
-                    float2* dst = land + l * C::LANDW;
-                    // 16-byte chunk q of the compact line: quarter q % 4 of the 64-byte piece in tile q / 4
-                    for (int q = lane; q < xb; q += 32)
-                        cp_async16(dst + 2 * q, src + (size_t)(q >> 2) * g.ny * 8 + 2 * (q & 3));
-                }
-            }
-            cp_async_arrive(&bars[warp]);
-        } else {
-            int n_act = 0;
+        for (int l = 0; l < LPW; ++l) n_act += (w0 + l < g.n_waves);
+        mbar_expect_tx(&bars[warp], (unsigned)(n_act * 2 * xb * (int)sizeof(float2)));
 #pragma unroll
-            for (int l = 0; l < LPW; ++l) n_act += (w0 + l < g.n_waves);
-            mbar_expect_tx(&bars[warp], (unsigned)(n_act * 2 * xb * (int)sizeof(float2)));
-#pragma unroll
-            for (int l = 0; l < LPW; ++l)
-                if (w0 + l < g.n_waves) tensor_g2s_4d(land + l * C::LANDW, &tmap, 0, y, 0, w0 + l, &bars[warp]);
-        }
+        for (int l = 0; l < LPW; ++l)
+            if (w0 + l < g.n_waves) tensor_g2s_4d(land + l * C::LANDW, &tmap, 0, y, 0, w0 + l, &bars[warp]);
     };
-    if (MODE != ROW_INIT && (LOADER == LAY_B8_CPA || lane == 0) && my_lines > 0) issue(0);
+    if (MODE != ROW_INIT && lane == 0 && my_lines > 0) issue(0);
 
     const pk::XchgPhase sm{ xch + ll * P::XPAD, 1 };
     auto sync = [] { __syncwarp(); };
@@ -367,11 +347,7 @@ __global__ void __launch_bounds__(RowB8Cfg<N, XBE>::THREADS, 1) row_b8_kernel(Ro
             C2 p[32];
 
             constexpr int PH0 = (MODE == ROW_INIT) ? 1 : 0, PH1 = (MODE == ROW_FINAL) ? 1 : 2;
-#if PRISM_B8_ROW_UNROLL_PH
-#pragma unroll
-#else
 #pragma unroll 1
-#endif
             for (int ph = PH0; ph < PH1; ++ph) {
                 if (ph == 0) {
                     float2 v[64];
@@ -389,10 +365,7 @@ __global__ void __launch_bounds__(RowB8Cfg<N, XBE>::THREADS, 1) row_b8_kernel(Ro
                     }
                     // the landing buffer is free once every lane has read its points
                     __syncwarp();
-                    if (seq + 1 < my_lines) {
-                        if (LOADER == LAY_B8_CPA) issue(seq + 1);
-                        else if (lane == 0) { fence_proxy_async(); issue(seq + 1); }
-                    }
+                    if (seq + 1 < my_lines && lane == 0) { fence_proxy_async(); issue(seq + 1); }
                     pk::dif_pre<P, XBE, true>(v, p, tab, t);       // inverse = conj of the forward transform of conj(v)
                 } else {
                     if (MODE == ROW_INIT) {
@@ -483,15 +456,11 @@ static cudaError_t encode_line_map(const RowArgs& g, CUtensorMap* map)
     return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
 }
 
-#ifndef PRISM_B8_ROW_LOADER
-#define PRISM_B8_ROW_LOADER LAY_B8_TMA
-#endif
-
 template <int N, int MODE, int XBE>
 static cudaError_t launch_row_b8_x(const RowArgs& g, cudaStream_t stream)
 {
     using C = RowB8Cfg<N, XBE>;
-    auto kern = row_b8_kernel<N, MODE, XBE, PRISM_B8_ROW_LOADER>;
+    auto kern = row_b8_kernel<N, MODE, XBE>;
     static PerDevice once{};
     if (cudaError_t e = opt_in_smem(kern, C::SMEM, once); e != cudaSuccess) return e;
     if (g.n_waves <= 0) return cudaSuccess;
@@ -501,7 +470,7 @@ static cudaError_t launch_row_b8_x(const RowArgs& g, cudaStream_t stream)
     if (grid > g.ny) grid = g.ny;
     CUtensorMap map;
     std::memset(&map, 0, sizeof(map));
-    if (PRISM_B8_ROW_LOADER == LAY_B8_TMA && MODE != ROW_INIT)
+    if (MODE != ROW_INIT)
         if (cudaError_t e = encode_line_map(g, &map); e != cudaSuccess) return e;
     return launch_pdl(kern, (unsigned)grid, C::THREADS, C::SMEM, stream, g, map);
 }

@@ -18,9 +18,7 @@
 // The transforms and the summation order are those of row_pass_kernel / col_pass_kernel / bin_reduce_kernel
 // (slice_pass.cu, output.cu), which this kernel replaces on the PRISM output path.
 // complex adds of the register butterflies as packed FADD2: the kernel is bound by issue slots (16 warps per SM)
-#ifndef PRISM_WINDOW_SCALAR_ADDS
 #define PRISM_PACKED_ADDS 1
-#endif
 #include "fft_core.cuh"
 #include "prism_internal.h"
 

@@ -13,8 +13,7 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-# PRISM_B200_LIB: load a variant build of the library (build.build(extra_flags=..., lib_path=...)) instead
-LIB_PATH = os.environ.get("PRISM_B200_LIB") or os.path.join(_HERE, "libprism_b200.so")
+LIB_PATH = os.path.join(_HERE, "libprism_b200.so")
 
 PRISM_OK, PRISM_EINVAL, PRISM_ENOMEM, PRISM_ECUDA, PRISM_EUNSUPPORTED, PRISM_ENOLUT = 0, -1, -2, -3, -4, -5
 WS_SMATRIX, WS_OUTPUT, WS_MULTISLICE, WS_POTENTIAL, WS_MULTISLICE_PATTERNS = 0, 1, 2, 3, 4
