@@ -173,7 +173,9 @@ int prism_build_potential_static(const prism_params* p, const double* atoms_xyz,
  * band-limit on P), and its real-space exit wave stored as layer b at full resolution (R17).
  *   v      IN   [n_slices][ny][nx] fp32, device or page-locked host (potential_on_host)
  *   beams  OUT  HOST [n_beams][2] int32 (kx, ky) of each layer, n_beams from prism_num_beams
- *   s      OUT  DEVICE complex64 [n_beams][ny][nx]; also the working set (waves are updated in place)
+ *   s      OUT  complex64 [n_beams][ny][nx].  smatrix_on_host = 0: DEVICE memory, also the working set (waves are
+ *               updated in place).  smatrix_on_host = 1: PAGE-LOCKED HOST memory; `batch` beams at a time are
+ *               propagated in the workspace and their layers copied out
  *   workspace DEVICE, prism_workspace_bytes(p, PRISM_WS_SMATRIX) */
 int prism_compute_smatrix(const prism_params* p, const float* v, int32_t* beams, void* s,
                           void* workspace, size_t workspace_bytes, void* cuda_stream);
@@ -181,7 +183,7 @@ int prism_compute_smatrix(const prism_params* p, const float* v, int32_t* beams,
 /* PRISM probes (Fig. 1i-k): for every probe of the grid, the (nx/f) x (ny/f) window of
  * every layer around the probe is weighted by A_b exp(-i chi_b) exp(-2 pi i q_b . r_p) / (sqrt(n_beams)
  * sqrt(mx my)) and summed over beams, Fourier transformed, squared (/ (mx my)) and integrated into rings.
- *   s      IN   DEVICE complex64 [n_beams][ny][nx]      beams  IN  HOST [n_beams][2]
+ *   s      IN   complex64 [n_beams][ny][nx], DEVICE (page-locked HOST if smatrix_on_host)      beams  IN  HOST [n_beams][2]
  *   out    OUT  fp32 [probes_y][probes_x][n_bins]; device memory or host memory (then copied inside the call)
  *   workspace DEVICE, prism_workspace_bytes(p, PRISM_WS_OUTPUT) */
 int prism_compute_output(const prism_params* p, const void* s, const int32_t* beams, int32_t n_beams,
