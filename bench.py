@@ -295,7 +295,7 @@ def run_multislice(args, name, steps, warmup):
     e2e_s = time.perf_counter() - t0
     hbm_peak, peak_src = measured_peaks()
     batch = w.batch if w.batch > 0 else n_probes
-    band = 2.0 * prism.band_columns(p) / w.nx if min(w.nx, w.ny) >= 256 else 1.0
+    band = 2.0 / 3.0 if min(w.nx, w.ny) >= 256 else 1.0                 # the in-band 2/3 of mixed space
     per_launch = 16.0 * npix * band * min(batch, n_probes)              # one pass over one batch of probes
     kernels = {}
     for kname, (ms, cnt) in kern.items():
@@ -476,7 +476,13 @@ def run_prism(name, steps, warmup, world, rank, local, dist, want_cpu_baseline, 
     m2 = (w.nx // w.f) * (w.ny // w.f)
     # algorithmic bytes per wave and pass: mixed space is moved for the 2c in-band columns of
     # the nx only (c = prism_band_columns; whole waves below 256 points), real space in full
-    band = 2.0 * prism.band_columns(p) / w.nx if min(w.nx, w.ny) >= 256 else 1.0
+    # The ALGORITHMIC band is SURVEY.md 8(d)'s: the in-band 2/3 of each mixed-space row (21.3 N^2 bytes per beam-slice
+    # for the two passes).  The kernels move the band rounded up to whole 32-column groups (`band_moved`, 0.6875 at
+    # 2048, 0.75 at 512): those extra columns are not counted as useful bytes; fractions on the moved bytes are
+    # reported beside, under "moved_band".
+    banded = min(w.nx, w.ny) >= 256
+    band = 2.0 / 3.0 if banded else 1.0
+    band_moved = 2.0 * prism.band_columns(p) / w.nx if banded else 1.0
     mixed, real = 8 * npix * n_beams * band, 8 * npix * n_beams
     # algorithmic bytes per step and kernel class (a class may be split over several launches: the blocked layout runs
     # ROW_FINAL a few waves at a time)
@@ -488,17 +494,32 @@ def run_prism(name, steps, warmup, world, rank, local, dist, want_cpu_baseline, 
         if kname in per_step_bytes:
             entry["algorithmic_GBps"] = per_step_bytes[kname] / (ms / inst_steps * 1e-3) / 1e9
             entry["frac_of_hbm_peak"] = entry["algorithmic_GBps"] / hbm_peak
+            if kname != "row_final":
+                entry["frac_moved_band"] = entry["frac_of_hbm_peak"] * band_moved / band
         if kname == "beam_sum":
+            # fallback for probe sets that are not a regular lattice: one CTA per probe re-reads its windows of every
+            # layer (L2 / HBM): 8 N_b M^2 bytes and 8 N_b M^2 flop per probe
             entry["algorithmic_TFLOPs"] = 8.0 * n_beams * m2 * n_probes * inst_steps / (ms * 1e-3) / 1e12
+            entry["window_read_GBps"] = 8.0 * n_beams * m2 * n_probes * inst_steps / (ms * 1e-3) / 1e9
+            entry["frac_of_hbm_peak"] = entry["window_read_GBps"] / hbm_peak
+            entry["fp32_frac"] = entry["algorithmic_TFLOPs"] / FP32_PEAK_TFLOPS
         # stage 2: the lattice kernel reads the pixel rows of a probe-row batch once and writes
         # the summed windows; window_out reads every window once
         if kname == "lattice_dft":
             sy = max(1, int(round(w.probe_step[1] / (w.cell[1] / w.ny))))
             rows_per_launch = max(1, int(round(w.probes_y * inst_steps / cnt)))
             pix_rows = min(w.ny, sy * (rows_per_launch - 1) + w.ny // w.f)
-            lat_bytes = (cnt / inst_steps) * 8.0 * n_beams * pix_rows * w.nx + 8.0 * m2 * n_probes
+            # algorithmic: ONE read of the pixel rows the probe grid's windows cover + the summed windows written once.
+            # Rows shared by consecutive probe-row batches are read again by each batch (the batch is sized by the
+            # workspace): that re-read is reported as its own factor, not counted as useful bytes.
+            rows_once = min(w.ny, sy * (w.probes_y - 1) + w.ny // w.f)
+            rows_read = (cnt / inst_steps) * pix_rows
+            lat_bytes = 8.0 * n_beams * rows_once * w.nx + 8.0 * m2 * n_probes
             entry["algorithmic_GBps"] = lat_bytes / (ms / inst_steps * 1e-3) / 1e9
             entry["frac_of_hbm_peak"] = entry["algorithmic_GBps"] / hbm_peak
+            entry["batch_reread_factor"] = rows_read / rows_once
+            entry["frac_incl_batch_rereads"] = ((8.0 * n_beams * rows_read * w.nx + 8.0 * m2 * n_probes)
+                                                / (ms / inst_steps * 1e-3) / 1e9 / hbm_peak)
         if kname == "window_out":
             entry["algorithmic_GBps"] = 8.0 * m2 * n_probes / (ms / inst_steps * 1e-3) / 1e9
             entry["frac_of_hbm_peak"] = entry["algorithmic_GBps"] / hbm_peak
@@ -510,7 +531,11 @@ def run_prism(name, steps, warmup, world, rank, local, dist, want_cpu_baseline, 
         ach = kernels[top]["algorithmic_GBps"]
         roofline = {"kernel": top, "bound": "hbm", "achieved": ach, "peak": hbm_peak, "unit": "GB/s",
                     "frac": ach / hbm_peak, "traffic": measured_traffic(w.name, top), "peak_source": peak_src,
-                    "bytes_per_launch": per_step_bytes[top] / kernels[top]["launches_per_step"]}
+                    "bytes_per_launch": per_step_bytes[top] / kernels[top]["launches_per_step"],
+                    "bytes_assume": ("SURVEY.md 8(d): 2/3 of each mixed-space row in and out per pass "
+                                     "(10.67 N^2 bytes per wave and pass)" if banded else "whole waves (grid < 256)"),
+                    "moved_band": {"band_fraction": band_moved, "frac": ach / hbm_peak * band_moved / band,
+                                   "bytes_per_launch": per_step_bytes[top] / kernels[top]["launches_per_step"] * band_moved / band}}
     else:
         ach = kernels[top].get("algorithmic_TFLOPs", 0.0)
         roofline = {"kernel": top, "bound": "alu", "achieved": ach, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
@@ -521,7 +546,7 @@ def run_prism(name, steps, warmup, world, rank, local, dist, want_cpu_baseline, 
     flops = n_beams * w.n_slices * npix * (10.0 * (np.log2(w.nx) + np.log2(w.ny)) + 12.0)
     roofline["slice_step"] = {"algorithmic_GBps": step_bytes / (slice_ms * 1e-3) / 1e9,
                               "frac": step_bytes / (slice_ms * 1e-3) / 1e9 / hbm_peak,
-                              "band_fraction": band,
+                              "band_fraction": band, "band_fraction_moved": band_moved,
                               "unbanded_32N2_GBps": 32.0 * npix * n_beams * w.n_slices / (slice_ms * 1e-3) / 1e9,
                               "fp32_TFLOPs_nominal": flops / (slice_ms * 1e-3) / 1e12,
                               "fp32_frac": flops / (slice_ms * 1e-3) / 1e12 / FP32_PEAK_TFLOPS}
